@@ -1,0 +1,316 @@
+#!/usr/bin/env python
+"""bench.py — headline measurement of the H / H^T pair.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config k]
+
+One "step" = one pass of the whole hot path on one workload: data = H p0 followed by
+image = H^T data (a single gradient evaluation) on BASELINE.json config 4 (512^3, 4000 samples,
+4096 receivers) unless --config says otherwise.  Metric: Gcell-updates/s, where one call of H or
+H^T performs nx*ny*nz*(nt-1) cell updates.  For N > 1 (torchrun) every rank runs an independent
+replica of the workload on its own GPU ("replicas only"): value = all ranks' cell
+updates / max-over-ranks device time.
+
+Prints ONE JSON line on rank 0.  `--impl reference` times the fp64 CPU oracle instead (rank 0).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "Gcell-updates/s for elastic FDTD forward+adjoint"
+UNIT = "Gcell-updates/s"
+B_ALG = 88.0          # algorithmic bytes per cell per time step (9 state R+W, 4 materials R)
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config (1-based); 4 is the headline")
+    ap.add_argument("--nt", type=int, default=None, help="development only: truncate the number of samples")
+    ap.add_argument("--variant", type=int, default=0, help="kernel variant (0 = library default)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+# ---------------------------------------------------------------------------------------------
+def workload_name(prob, args):
+    p = prob.prm
+    s = f"BASELINE config {args.config}: {p.nx}x{p.ny}x{p.nz}, nt={p.nt}, L={prob.L}, npml={p.npml}"
+    if args.nt is not None:
+        s += " (nt truncated: development run, not the headline)"
+    return s
+
+
+def cpu_sample(prob):
+    """Bounded sample of the workload for the oracle: a block of the same volumes, few samples."""
+    from paper_1709_02733_b200 import synth
+    n_full = prob.prm.nx
+    n = min(n_full, 160)
+    nt = 12 if n_full > n else min(prob.prm.nt, 12)
+    if n_full > n:
+        # block under the top of the hemispherical array: contains water, porous skull and receivers
+        x0 = y0 = (n_full - n) // 2
+        z0 = n_full - n - max(prob.prm.npml // 2, 1)
+        sub = synth.crop(prob, (x0, y0, z0), n, nt)
+        what = f"{n}^3 block at ({x0},{y0},{z0}) of the workload's volumes, nt={nt}, {sub.L} receivers, forward+adjoint"
+    else:
+        from dataclasses import replace
+        sub = replace(prob, prm=replace(prob.prm, nt=nt))
+        what = f"the full {n}^3 grid, nt={nt}, forward+adjoint"
+    return sub, what
+
+
+def time_oracle(sub, repeats=2):
+    """Seconds for one forward + one adjoint of the oracle on `sub` (as it stands, OpenMP threads);
+    best of `repeats` (the first pass also pays page faults and thread start-up)."""
+    import numpy as np
+    from oracle.oracle import Oracle, threads
+    o = Oracle.from_problem(sub)
+    p0 = sub.p0.astype(np.float64)
+    best = float("inf")
+    for _ in range(repeats):
+        t = time.perf_counter()
+        d = o.forward(p0)
+        o.adjoint(d)
+        best = min(best, time.perf_counter() - t)
+    o.close()
+    cells = 2.0 * sub.prm.N * (sub.prm.nt - 1)
+    return best, cells, threads()
+
+
+def run_reference(args):
+    """`--impl reference`: the fp64 CPU oracle on a bounded sample of the arm's workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_1709_02733_b200 import synth
+    prob = synth.make_config(args.config, nt=args.nt)
+    sub, what = cpu_sample(prob)
+    for _ in range(max(args.warmup, 0) and 1):
+        time_oracle(sub)
+    t_tot, cells_tot = 0.0, 0.0
+    cores = 1
+    for _ in range(max(args.steps, 1)):
+        t, cells, cores = time_oracle(sub)
+        t_tot += t
+        cells_tot += cells
+    v = cells_tot / t_tot / 1e9
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_tot / max(args.steps, 1),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(prob, args), "sample": what},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ---------------------------------------------------------------------------------------------
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.path = index, None, None
+
+    def start(self):
+        try:
+            f = tempfile.NamedTemporaryFile("w", suffix=".csv", delete=False)
+            self.path = f.name
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"], stdout=f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if not self.proc:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, smax, reasons = [], [], set()
+        try:
+            for ln in open(self.path):
+                c = [v.strip() for v in ln.split(",")]
+                if len(c) < 9:
+                    continue
+                try:
+                    sm.append(float(c[1])); smax.append(float(c[2]))
+                except ValueError:
+                    continue
+                for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), c[5:9]):
+                    if v.lower().startswith("active"):
+                        reasons.add(name)
+            os.unlink(self.path)
+        except Exception:
+            pass
+        if sm:
+            sm.sort()
+            out.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=max(smax), samples=len(sm))
+        out["reasons"] = sorted(reasons)
+        return out
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+        return
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_1709_02733_b200 import build, synth
+    from paper_1709_02733_b200.binding import Pact
+
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    build.build()
+
+    prob = synth.make_config(args.config, nt=args.nt)     # every rank: an independent replica
+    prm = prob.prm
+    ctx = Pact.from_problem(prob, device=dev)
+    ctx.set_option("variant", args.variant)
+    p0 = torch.from_numpy(prob.p0).to(dev)
+    data = torch.empty((prm.nt, prob.L), dtype=torch.float32, device=dev)
+    image = torch.empty(ctx.shape, dtype=torch.float32, device=dev)
+
+    def step():
+        ctx.forward(p0, out=data)        # data = H p0
+        ctx.adjoint(data, out=image)     # image = H^T data
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    ctx.set_option("profile", 1)         # CUDA events around sampled launches, on the library's stream
+    clocks = ClockSampler(local)
+    if rank == 0:
+        clocks.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize(dev)
+    ev0.record(ctx.stream)
+    for _ in range(args.steps):
+        step()
+    ev1.record(ctx.stream)
+    torch.cuda.synchronize(dev)
+    barrier()
+    clk = clocks.stop() if rank == 0 else None
+    ms = torch.tensor([ev0.elapsed_time(ev1)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+    ms = float(ms.item())
+    cells_step = 2.0 * prm.N * (prm.nt - 1)                # forward + adjoint
+    value = world * cells_step * args.steps / (ms * 1e-3) / 1e9
+
+    # ---- roofline of the step kernels, from the library's own CUDA events in the timed region
+    loop_f, k_f, n_f = ctx.timing("forward")
+    loop_a, k_a, n_a = ctx.timing("adjoint")
+    ctx.set_option("profile", 0)
+    launches = (sum(n_f.values()) + sum(n_a.values()) + 4) * args.steps   # + argument record x2, tau, tau^T per step
+    # device time of one time step's kernels (all launches of the step, in the mix they ran)
+    t_fwd = (k_f["fwd_vel"] * n_f["fwd_vel"] + k_f["fwd_str"] * n_f["fwd_str"] + k_f["fwd_fused"] * n_f["fwd_fused"]) / max(prm.nt - 1, 1)
+    t_adj = (k_a["adj_a"] * n_a["adj_a"] + k_a["adj_b"] * n_a["adj_b"] + k_a["adj_fused"] * n_a["adj_fused"]) / max(prm.nt - 1, 1)
+    peak, peak_src = peaks()
+    pml_extra = 48.0 * 3 * 2 * prm.npml / prm.nx if prm.npml else 0.0
+    roof = None
+    if t_fwd > 0 and t_adj > 0:
+        ach = 2 * B_ALG * prm.N / ((t_fwd + t_adj) * 1e-3) / 1e9
+        roof = {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
+                "peak_source": peak_src, "kernel": "step kernels of one forward + one adjoint time step",
+                "bytes_per_cell_step": B_ALG, "pml_bytes_per_cell_step_not_credited": pml_extra,
+                "forward_step_ms": t_fwd, "adjoint_step_ms": t_adj,
+                "forward_frac": B_ALG * prm.N / (t_fwd * 1e-3) / 1e9 / peak,
+                "adjoint_frac": B_ALG * prm.N / (t_adj * 1e-3) / 1e9 / peak,
+                "forward_loop_ms": loop_f, "adjoint_loop_ms": loop_a,
+                "kernel_ms": {"forward": {k: v for k, v in k_f.items() if v}, "adjoint": {k: v for k, v in k_a.items() if v}}}
+        tr = os.path.join(ROOT, "profiles", "traffic.json")   # per-launch DRAM bytes from the committed ncu capture
+        if os.path.exists(tr):
+            try:
+                roof["traffic"] = json.load(open(tr)).get(f"config{args.config}")
+            except Exception:
+                pass
+
+    # ---- end to end through the host-buffer entry points (pinned host memory, copies inside)
+    e2e = None
+    if not args.no_e2e:
+        p0_h = torch.from_numpy(prob.p0).pin_memory()
+        data_h = torch.empty((prm.nt, prob.L), dtype=torch.float32).pin_memory()
+        image_h = torch.empty(ctx.shape, dtype=torch.float32).pin_memory()
+        n_e2e = 1
+        ctx.forward_host(p0_h, data_h); ctx.adjoint_host(data_h, image_h)     # warm (staging buffers)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            ctx.forward_host(p0_h, data_h)
+            ctx.adjoint_host(data_h, image_h)
+        torch.cuda.synchronize(dev)
+        t_e = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t_e, op=dist.ReduceOp.MAX)
+        nb = prm.N * 4 + prm.nt * prob.L * 4
+        e2e = {"value": world * cells_step * n_e2e / float(t_e.item()) / 1e9, "unit": UNIT,
+               "h2d_bytes_per_step": nb, "d2h_bytes_per_step": nb, "steps": n_e2e,
+               "api": "pact_forward_host + pact_adjoint_host (pinned host buffers)"}
+
+    # ---- the oracle beside it (rank 0, N = 1 only)
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        sub, what = cpu_sample(prob)
+        t, cells, cores = time_oracle(sub)
+        cpu = {"value": cells / t / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": what, "seconds": t}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": workload_name(prob, args), "parallelism": "replicas only" if world > 1 else "single GPU",
+                           "step": "one pact_forward + one pact_adjoint", "l2": "inputs larger than L2 (no flush needed)"
+                           if ctx.device_bytes() > 4 * 126e6 else "working set near L2 size: latency/L2-bound case",
+                           "variant": args.variant, "device_bytes": ctx.device_bytes()},
+                "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clk}
+        print(json.dumps(line), flush=True)
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,572 @@
+// pact.cu — host side of libpact: the C ABI of include/pact.h.
+//
+// Everything numerical happens in the kernels of kernels_*.cuh; this file validates arguments,
+// derives the tables that depend only on the parameters (C-PML profiles, trilinear rows), owns the
+// device buffers and enqueues the time loops of Eq. 58 (forward) and Eq. 59/27 (adjoint).
+// There is no CPU fallback: every entry point either enqueues CUDA work or returns an error.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "../../include/pact.h"
+#include "common.cuh"
+#include "kernels_io.cuh"
+#include "kernels_plain.cuh"
+#include "kernels_tiled.cuh"
+
+// ------------------------------------------------------------------------------------------------
+static thread_local char g_cuda_err[512] = "";
+
+static int cuda_fail(cudaError_t e, const char* what, int line)
+{
+    snprintf(g_cuda_err, sizeof(g_cuda_err), "%s (pact.cu:%d): %s", what, line, cudaGetErrorString(e));
+    return e == cudaErrorMemoryAllocation ? PACT_ENOMEM : PACT_ECUDA;
+}
+#define CK(call)                                                          \
+    do {                                                                  \
+        cudaError_t e_ = (call);                                          \
+        if (e_ != cudaSuccess) return cuda_fail(e_, #call, __LINE__);     \
+    } while (0)
+
+#define MAX_SAMPLES 48
+
+struct EvPair { cudaEvent_t a, b; };
+
+struct pact_ctx {
+    pact_params prm;
+    cudaStream_t stream;
+    long long N;             // nx ny nz
+    int L;
+    int pitch, py, pz;       // padded box extents
+    long long box;           // elements of one padded field
+    DevGrid g;
+    RcvTables rcv;
+    IoArgs* d_io;
+    std::vector<void*> allocs;
+    long long bytes;
+    // zeroed at the start of every operator call: state fields + memory variables (contiguous)
+    float* state_base;
+    long long state_bytes;
+    float* scratch_base;     // adjoint scratch of the plain variant, allocated on first use
+    // host-buffer variants
+    float* d_vol;            // [N]
+    float* d_dat;            // [nt][L]
+    // options
+    int variant;             // 0 auto, 1 plain, 2 tiled
+    int use_graph;           // -1 auto, 0 off, 1 on
+    int profile;
+    cudaGraphExec_t gexec[2];     // forward / adjoint loop
+    int gexec_variant[2];
+    // timing of the last profiled call
+    // timing of the last profiled forward ([0]) / adjoint ([1]) call
+    cudaEvent_t ev_loop[2][2];
+    std::vector<EvPair> samples[2][8];
+    size_t used[2][8];
+    long long launches[2][8];
+    bool have_timing[2];
+};
+
+static int dev_alloc(pact_ctx* c, void** p, size_t bytes)
+{
+    if (bytes == 0) bytes = 16;
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e != cudaSuccess) { *p = nullptr; return cuda_fail(e, "cudaMalloc", __LINE__); }
+    c->allocs.push_back(*p);
+    c->bytes += (long long)bytes;
+    return PACT_OK;
+}
+
+template <typename T>
+static int upload(pact_ctx* c, T** dst, const std::vector<T>& v)
+{
+    int rc = dev_alloc(c, (void**)dst, v.size() * sizeof(T));
+    if (rc) return rc;
+    if (!v.empty()) CK(cudaMemcpyAsync(*dst, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaStreamSynchronize(c->stream));   // v may be a temporary
+    return PACT_OK;
+}
+
+// ---- C-PML profiles, Eq. 38 with kappa = 1; profile shape: DESIGN.md reading G8
+//   depth = max(P - s, s - (n-1-P), 0) cells, xi = depth/P, d = d0 xi^2, d0 = -3 c_ref ln R/(2 P h),
+//   beta = beta_max (1 - xi);  b = exp(-(d + beta) dt),  a = d/(d + beta) (b - 1), a = 0 where d = 0.
+static void cpml_profile(const pact_params& p, int n, bool half, std::vector<float>& a, std::vector<float>& b)
+{
+    a.assign(n, 0.0f);
+    b.assign(n, 1.0f);
+    const int P = p.npml;
+    if (P <= 0) return;
+    const double d0 = -3.0 * p.pml_cref * std::log(p.pml_R) / (2.0 * P * p.h);
+    for (int i = 0; i < n; ++i) {
+        const double s = i + (half ? 0.5 : 0.0);
+        const double depth = std::max(std::max((double)P - s, s - (double)(n - 1 - P)), 0.0);
+        if (depth <= 0.0) continue;
+        const double xi = depth / P;
+        const double d = d0 * xi * xi, beta = p.pml_beta_max * (1.0 - xi);
+        const double bb = std::exp(-(d + beta) * p.dt);
+        b[i] = (float)bb;
+        a[i] = d > 0.0 ? (float)(d / (d + beta) * (bb - 1.0)) : 0.0f;
+    }
+}
+
+static void free_graphs(pact_ctx* c)
+{
+    for (int k = 0; k < 2; ++k)
+        if (c->gexec[k]) { cudaGraphExecDestroy(c->gexec[k]); c->gexec[k] = nullptr; }
+}
+
+extern "C" void pact_destroy(pact_ctx* c)
+{
+    if (!c) return;
+    cudaStreamSynchronize(c->stream);
+    free_graphs(c);
+    for (int op = 0; op < 2; ++op) {
+        for (int k = 0; k < 8; ++k)
+            for (auto& s : c->samples[op][k]) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
+        for (int k = 0; k < 2; ++k) if (c->ev_loop[op][k]) cudaEventDestroy(c->ev_loop[op][k]);
+    }
+    for (void* p : c->allocs) cudaFree(p);
+    delete c;
+}
+
+extern "C" const char* pact_strerror(int code)
+{
+    switch (code) {
+    case PACT_OK: return "ok";
+    case PACT_EINVAL: return "invalid argument";
+    case PACT_ECFL: return "time step exceeds the stability limit dt*c_max <= 6h/(7 sqrt 3)";
+    case PACT_ERCV: return "receiver outside the grid";
+    case PACT_EMATERIAL: return "invalid material value";
+    case PACT_ENOMEM: return "out of memory";
+    case PACT_ECUDA: return "CUDA error";
+    default: return "unknown error";
+    }
+}
+
+extern "C" const char* pact_last_cuda_error(void) { return g_cuda_err; }
+
+extern "C" long long pact_device_bytes(const pact_ctx* c) { return c ? c->bytes : 0; }
+
+// ------------------------------------------------------------------------------------------------
+// pact_create
+static int create_impl(pact_ctx* c, const pact_params* prm, const float* lam, const float* mu,
+                       const float* rho, const float* alpha, const double* rcv_xyz, int L)
+{
+    const int nx = prm->nx, ny = prm->ny, nz = prm->nz, P = prm->npml;
+    c->N = (long long)nx * ny * nz;
+    c->L = L;
+    c->pitch = ((nx + PACT_HALO_X + 4 + 31) / 32) * 32;
+    c->py = ny + 2 * PACT_HALO_Y;
+    c->pz = nz + 2 * PACT_HALO_Z;
+    c->box = (long long)c->pitch * c->py * c->pz;
+    DevGrid& g = c->g;
+    g.nx = nx; g.ny = ny; g.nz = nz; g.P = P; g.W = P > 0 ? 2 * P + 1 : 0;
+    g.sy = c->pitch; g.sz = (long long)c->pitch * c->py;
+    const long long org = (long long)PACT_HALO_Z * g.sz + (long long)PACT_HALO_Y * g.sy + PACT_HALO_X;
+
+    // ---- 1. scan the caller's volumes: validity and c_max (stability bound, reading G11)
+    unsigned int* d_scan = nullptr;
+    int rc = dev_alloc(c, (void**)&d_scan, 2 * sizeof(unsigned int));
+    if (rc) return rc;
+    CK(cudaMemsetAsync(d_scan, 0, 2 * sizeof(unsigned int), c->stream));
+    k_scan_materials<<<148 * 8, 256, 0, c->stream>>>(lam, mu, rho, alpha, c->N, d_scan, d_scan + 1);
+    CK(cudaGetLastError());
+    unsigned int h_scan[2];
+    CK(cudaMemcpyAsync(h_scan, d_scan, sizeof(h_scan), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    if (h_scan[0]) return PACT_EMATERIAL;
+    float c2;
+    memcpy(&c2, &h_scan[1], sizeof(float));
+    const double cmax = std::sqrt((double)c2);
+    const double limit = 6.0 * prm->h / (7.0 * std::sqrt(3.0));   // DESIGN.md reading G11
+    if (prm->dt * cmax > limit * (1.0 + 1e-6)) return PACT_ECFL;
+
+    // ---- 2. receivers: trilinear rows R_l and their node-sorted transpose
+    std::vector<long long> node8((size_t)8 * L);
+    std::vector<float> w8((size_t)8 * L);
+    {
+        const int n[3] = {nx, ny, nz};
+        for (int l = 0; l < L; ++l) {
+            int i0[3];
+            double t[3];
+            for (int b = 0; b < 3; ++b) {
+                double f = rcv_xyz[3 * l + b] / prm->h;
+                if (!(f >= -1e-9) || !(f <= (double)(n[b] - 1) + 1e-9)) return PACT_ERCV;
+                f = std::min(std::max(f, 0.0), (double)(n[b] - 1));
+                int i = (int)std::floor(f);
+                i = std::min(std::max(i, 0), n[b] - 2);
+                i0[b] = i;
+                t[b] = f - i;
+            }
+            for (int k = 0; k < 8; ++k) {
+                const int cx = k & 1, cy = (k >> 1) & 1, cz = (k >> 2) & 1;
+                node8[8 * l + k] = (long long)(i0[2] + cz) * g.sz + (long long)(i0[1] + cy) * g.sy + (i0[0] + cx);
+                w8[8 * l + k] = (float)((cx ? t[0] : 1.0 - t[0]) * (cy ? t[1] : 1.0 - t[1]) * (cz ? t[2] : 1.0 - t[2]));
+            }
+        }
+    }
+    std::vector<long long> tnode;
+    std::vector<int> row_ptr(1, 0), trcv;
+    std::vector<float> tw;
+    {
+        std::vector<std::pair<long long, int>> e((size_t)8 * L);   // (node, entry id) ; entry id = 8 l + k
+        for (int q = 0; q < 8 * L; ++q) e[q] = {node8[q], q};
+        std::sort(e.begin(), e.end());   // by node, then by receiver (ascending): fixed summation order
+        for (size_t q = 0; q < e.size(); ++q) {
+            if (q == 0 || e[q].first != e[q - 1].first) {
+                if (q) row_ptr.push_back((int)q);
+                tnode.push_back(e[q].first);
+            }
+            trcv.push_back(e[q].second / 8);
+            tw.push_back(w8[e[q].second]);
+        }
+        if (!e.empty()) row_ptr.push_back((int)e.size());
+    }
+    c->rcv.L = L;
+    c->rcv.nnodes = (int)tnode.size();
+    long long* d_ll; float* d_f; int* d_i;
+    if ((rc = upload(c, &d_ll, node8))) return rc; c->rcv.node8 = d_ll;
+    if ((rc = upload(c, &d_f, w8))) return rc;     c->rcv.w8 = d_f;
+    if ((rc = upload(c, &d_ll, tnode))) return rc; c->rcv.tnode = d_ll;
+    if ((rc = upload(c, &d_i, row_ptr))) return rc; c->rcv.row_ptr = d_i;
+    if ((rc = upload(c, &d_i, trcv))) return rc;   c->rcv.trcv = d_i;
+    if ((rc = upload(c, &d_f, tw))) return rc;     c->rcv.tw = d_f;
+
+    // ---- 3. C-PML tables
+    for (int b = 0; b < 3; ++b) {
+        const int n = b == 0 ? nx : (b == 1 ? ny : nz);
+        std::vector<float> ai, bi, ah, bh;
+        cpml_profile(*prm, n, false, ai, bi);
+        cpml_profile(*prm, n, true, ah, bh);
+        float* d;
+        if ((rc = upload(c, &d, ai))) return rc; g.tab[b][T_A_INT] = d;
+        if ((rc = upload(c, &d, bi))) return rc; g.tab[b][T_B_INT] = d;
+        if ((rc = upload(c, &d, ah))) return rc; g.tab[b][T_A_HALF] = d;
+        if ((rc = upload(c, &d, bh))) return rc; g.tab[b][T_B_HALF] = d;
+    }
+
+    // ---- 4. scaled, padded material volumes
+    float* mat = nullptr;
+    if ((rc = dev_alloc(c, (void**)&mat, (size_t)c->box * 4 * sizeof(float)))) return rc;
+    float* Ll = mat + org; float* Mi = Ll + c->box; float* Rr = Mi + c->box; float* Aa = Rr + c->box;
+    {
+        dim3 blk(128), grd((c->pitch + 127) / 128, c->py, c->pz);
+        k_scale_materials<<<grd, blk, 0, c->stream>>>(lam, mu, rho, alpha, nx, ny, nz, g.sy, g.sz, c->pitch,
+                                                      Ll, Mi, Rr, Aa, prm->dt / prm->h, prm->dt);
+        CK(cudaGetLastError());
+    }
+    g.Ll = Ll; g.Mi = Mi; g.Rr = Rr; g.Aa = Aa;
+
+    // ---- 5. state fields + memory variables, one contiguous block (zeroed per call)
+    long long mv[3] = {0, 0, 0};
+    if (P > 0) {
+        mv[0] = (long long)g.W * ny * nz;
+        mv[1] = (long long)nx * g.W * nz;
+        mv[2] = (long long)nx * ny * g.W;
+    }
+    auto r32 = [](long long v) { return (v + 31) / 32 * 32; };
+    long long total = c->box * NFIELD;
+    for (int b = 0; b < 3; ++b) total += 6 * r32(mv[b]);
+    c->state_bytes = total * (long long)sizeof(float);
+    if ((rc = dev_alloc(c, (void**)&c->state_base, (size_t)c->state_bytes))) return rc;
+    for (int k = 0; k < NFIELD; ++k) g.f[k] = c->state_base + (long long)k * c->box + org;
+    {
+        float* p = c->state_base + c->box * NFIELD;
+        for (int a = 0; a < 3; ++a)
+            for (int b = 0; b < 3; ++b) { g.phi[3 * a + b] = p; p += r32(mv[b]); }
+        for (int a = 0; a < 3; ++a)
+            for (int b = 0; b < 3; ++b) { g.psi[3 * a + b] = p; p += r32(mv[b]); }
+    }
+    for (int k = 0; k < 9; ++k) g.scr[k] = nullptr;
+
+    if ((rc = dev_alloc(c, (void**)&c->d_io, sizeof(IoArgs)))) return rc;
+    CK(cudaMemsetAsync(c->d_io, 0, sizeof(IoArgs), c->stream));
+    for (int op = 0; op < 2; ++op)
+        for (int k = 0; k < 2; ++k) CK(cudaEventCreate(&c->ev_loop[op][k]));
+    CK(cudaStreamSynchronize(c->stream));   // the caller may free its volumes now
+    CK(cudaGetLastError());
+    return PACT_OK;
+}
+
+extern "C" int pact_create(pact_ctx** out, const pact_params* prm, const float* lam, const float* mu,
+                           const float* rho, const float* alpha, const double* rcv_xyz, int L, void* cuda_stream)
+{
+    if (out) *out = nullptr;
+    if (!out || !prm || !lam || !mu || !rho || L < 0 || (L > 0 && !rcv_xyz)) return PACT_EINVAL;
+    if (prm->nx < 8 || prm->ny < 8 || prm->nz < 8 || prm->nt < 1 || prm->npml < 0) return PACT_EINVAL;
+    if (!(prm->h > 0.0) || !(prm->dt > 0.0) || !std::isfinite(prm->h) || !std::isfinite(prm->dt)) return PACT_EINVAL;
+    if (2 * prm->npml + 8 > std::min(prm->nx, std::min(prm->ny, prm->nz))) return PACT_EINVAL;
+    if (prm->npml > 0 && (!(prm->pml_R > 0.0 && prm->pml_R < 1.0) || !(prm->pml_cref > 0.0) ||
+                          !(prm->pml_beta_max >= 0.0) || !std::isfinite(prm->pml_beta_max)))
+        return PACT_EINVAL;
+    if ((double)prm->nx * prm->ny * prm->nz > 2.0e9) return PACT_EINVAL;   // 32-bit cell counts inside kernels
+    pact_ctx* c = new (std::nothrow) pact_ctx();
+    if (!c) return PACT_ENOMEM;
+    c->prm = *prm;
+    c->stream = (cudaStream_t)cuda_stream;
+    c->variant = 0;
+    c->use_graph = -1;
+    int rc = create_impl(c, prm, lam, mu, rho, alpha, rcv_xyz, L);
+    if (rc != PACT_OK) { pact_destroy(c); return rc; }
+    *out = c;
+    return PACT_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// time loops
+__global__ void k_set_io(IoArgs* io, IoArgs v) { *io = v; }
+
+struct Launcher {
+    pact_ctx* c;
+    int op;          // 0 forward, 1 adjoint
+    bool sample;     // record events around the launches of this step
+    int err;
+    template <typename F>
+    void run(int kind, F&& launch)
+    {
+        if (err) return;
+        EvPair* ev = nullptr;
+        if (sample && c->used[op][kind] < MAX_SAMPLES) {
+            if (c->used[op][kind] == c->samples[op][kind].size()) {
+                EvPair p;
+                if (cudaEventCreate(&p.a) != cudaSuccess || cudaEventCreate(&p.b) != cudaSuccess) {
+                    err = cuda_fail(cudaGetLastError(), "cudaEventCreate", __LINE__);
+                    return;
+                }
+                c->samples[op][kind].push_back(p);
+            }
+            ev = &c->samples[op][kind][c->used[op][kind]++];
+            cudaEventRecord(ev->a, c->stream);
+        }
+        launch();
+        if (ev) cudaEventRecord(ev->b, c->stream);
+        c->launches[op][kind]++;
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) err = cuda_fail(e, "kernel launch", __LINE__);
+    }
+};
+
+static int resolve_variant(const pact_ctx* c) { return c->variant == 0 ? PACT_DEFAULT_VARIANT : c->variant; }
+
+static int ensure_scratch(pact_ctx* c)
+{
+    if (c->scratch_base) return PACT_OK;
+    int rc = dev_alloc(c, (void**)&c->scratch_base, (size_t)c->box * 9 * sizeof(float));
+    if (rc) return rc;
+    CK(cudaMemsetAsync(c->scratch_base, 0, (size_t)c->box * 9 * sizeof(float), c->stream));   // halo stays 0
+    const long long org = (long long)PACT_HALO_Z * c->g.sz + (long long)PACT_HALO_Y * c->g.sy + PACT_HALO_X;
+    for (int k = 0; k < 9; ++k) c->g.scr[k] = c->scratch_base + (long long)k * c->box + org;
+    return PACT_OK;
+}
+
+static void forward_step(pact_ctx* c, Launcher& ln, int variant)
+{
+    const DevGrid& g = c->g;
+    cudaStream_t st = c->stream;
+    if (variant == 2) {
+        tiled_forward_step(g, st, ln);
+        return;
+    }
+    dim3 blk(PLAIN_BX, PLAIN_BY, PLAIN_BZ);
+    dim3 grd((g.nx + PLAIN_BX - 1) / PLAIN_BX, (g.ny + PLAIN_BY - 1) / PLAIN_BY, (g.nz + PLAIN_BZ - 1) / PLAIN_BZ);
+    ln.run(PACT_K_FWD_VEL, [&] { k_fwd_vel<<<grd, blk, 0, st>>>(g); });
+    ln.run(PACT_K_FWD_STR, [&] { k_fwd_str<<<grd, blk, 0, st>>>(g); });
+}
+
+static void adjoint_step(pact_ctx* c, Launcher& ln, int variant)
+{
+    const DevGrid& g = c->g;
+    cudaStream_t st = c->stream;
+    if (variant == 2) {
+        tiled_adjoint_step(g, st, ln);
+        return;
+    }
+    dim3 blk(PLAIN_BX, PLAIN_BY, PLAIN_BZ);
+    dim3 grd((g.nx + PLAIN_BX - 1) / PLAIN_BX, (g.ny + PLAIN_BY - 1) / PLAIN_BY, (g.nz + PLAIN_BZ - 1) / PLAIN_BZ);
+    ln.run(PACT_K_ADJ_A, [&] { k_adj_a1<<<grd, blk, 0, st>>>(g); });
+    ln.run(PACT_K_ADJ_A, [&] { k_adj_a2<<<grd, blk, 0, st>>>(g); });
+    ln.run(PACT_K_ADJ_B, [&] { k_adj_b1<<<grd, blk, 0, st>>>(g); });
+    ln.run(PACT_K_ADJ_B, [&] { k_adj_b2<<<grd, blk, 0, st>>>(g); });
+}
+
+// Eq. 58 right to left: tau, then for m = 0..M-1 { Theta ; W' unless m = M-1 }
+static int enqueue_forward_loop(pact_ctx* c, bool profile, int variant)
+{
+    const DevGrid& g = c->g;
+    cudaStream_t st = c->stream;
+    const int nt = c->prm.nt;
+    Launcher ln{c, 0, false, 0};
+    const int every = std::max(1, (nt - 1) / MAX_SAMPLES);
+    const dim3 rblk(128), rgrd((c->L + 127) / 128);
+    for (int m = 0; m < nt; ++m) {
+        ln.sample = profile && (m % every == every / 2);
+        if (c->L > 0) ln.run(PACT_K_RECV, [&] { k_gather<<<rgrd, rblk, 0, st>>>(g, c->rcv, c->d_io, m); });
+        if (m < nt - 1) forward_step(c, ln, variant);
+    }
+    return ln.err;
+}
+
+// Eq. 27 / 60 with 27b's indexing (reading G4):
+//   v = 0 ; for m = M-1..0 { v <- W'^T v unless m = M-1 ; v += Theta'^T p^_m } ; image = tau^T v
+static int enqueue_adjoint_loop(pact_ctx* c, bool profile, int variant)
+{
+    const DevGrid& g = c->g;
+    cudaStream_t st = c->stream;
+    const int nt = c->prm.nt;
+    Launcher ln{c, 1, false, 0};
+    const int every = std::max(1, (nt - 1) / MAX_SAMPLES);
+    const dim3 rblk(128), rgrd((c->rcv.nnodes + 127) / 128);
+    for (int m = nt - 1; m >= 0; --m) {
+        ln.sample = profile && (m % every == every / 2);
+        if (m < nt - 1) adjoint_step(c, ln, variant);
+        if (c->L > 0) ln.run(PACT_K_RECV, [&] { k_scatter<<<rgrd, rblk, 0, st>>>(g, c->rcv, c->d_io, m); });
+    }
+    return ln.err;
+}
+
+static bool want_graph(const pact_ctx* c)
+{
+    if (c->profile) return false;
+    if (c->use_graph >= 0) return c->use_graph != 0;
+    // auto: small grids are launch-bound (a 64^3 step is a few microseconds); big ones are not
+    return c->N <= (1ll << 22) && c->prm.nt <= 4096;
+}
+
+static int run_loop(pact_ctx* c, int which /*0 fwd, 1 adj*/)
+{
+    const int variant = resolve_variant(c);
+    if (which == 1 && variant == 1) { int rc = ensure_scratch(c); if (rc) return rc; }
+    for (int k = 0; k < 8; ++k) { c->used[which][k] = 0; c->launches[which][k] = 0; }
+    c->have_timing[which] = c->profile != 0;
+    if (want_graph(c)) {
+        if (c->gexec[which] && c->gexec_variant[which] != variant) {
+            cudaGraphExecDestroy(c->gexec[which]);
+            c->gexec[which] = nullptr;
+        }
+        if (!c->gexec[which]) {
+            cudaGraph_t graph = nullptr;
+            CK(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+            int rc = which == 0 ? enqueue_forward_loop(c, false, variant) : enqueue_adjoint_loop(c, false, variant);
+            cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+            if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+            if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture", __LINE__);
+            e = cudaGraphInstantiate(&c->gexec[which], graph, 0);
+            cudaGraphDestroy(graph);
+            if (e != cudaSuccess) { c->gexec[which] = nullptr; return cuda_fail(e, "cudaGraphInstantiate", __LINE__); }
+            c->gexec_variant[which] = variant;
+        }
+        CK(cudaGraphLaunch(c->gexec[which], c->stream));
+        return PACT_OK;
+    }
+    if (c->profile) CK(cudaEventRecord(c->ev_loop[which][0], c->stream));
+    int rc = which == 0 ? enqueue_forward_loop(c, c->profile != 0, variant) : enqueue_adjoint_loop(c, c->profile != 0, variant);
+    if (rc) return rc;
+    if (c->profile) CK(cudaEventRecord(c->ev_loop[which][1], c->stream));
+    return PACT_OK;
+}
+
+extern "C" int pact_forward(pact_ctx* c, const float* p0, float* data)
+{
+    if (!c || !p0 || (!data && c->L > 0)) return PACT_EINVAL;
+    cudaStream_t st = c->stream;
+    IoArgs io{p0, data, nullptr, nullptr};
+    k_set_io<<<1, 1, 0, st>>>(c->d_io, io);
+    CK(cudaMemsetAsync(c->state_base, 0, (size_t)c->state_bytes, st));
+    dim3 blk(64, 4), grd((c->g.nx + 63) / 64, (c->g.ny + 3) / 4, c->g.nz);
+    k_inject<<<grd, blk, 0, st>>>(c->g, c->d_io);
+    CK(cudaGetLastError());
+    return run_loop(c, 0);
+}
+
+extern "C" int pact_adjoint(pact_ctx* c, const float* data, float* image)
+{
+    if (!c || !image || (!data && c->L > 0)) return PACT_EINVAL;
+    cudaStream_t st = c->stream;
+    IoArgs io{nullptr, nullptr, data, image};
+    k_set_io<<<1, 1, 0, st>>>(c->d_io, io);
+    CK(cudaMemsetAsync(c->state_base, 0, (size_t)c->state_bytes, st));
+    int rc = run_loop(c, 1);
+    if (rc) return rc;
+    dim3 blk(64, 4), grd((c->g.nx + 63) / 64, (c->g.ny + 3) / 4, c->g.nz);
+    k_image<<<grd, blk, 0, st>>>(c->g, c->d_io);
+    CK(cudaGetLastError());
+    return PACT_OK;
+}
+
+// ---- host-buffer variants -----------------------------------------------------------------------
+static int ensure_host_staging(pact_ctx* c)
+{
+    if (!c->d_vol) { int rc = dev_alloc(c, (void**)&c->d_vol, (size_t)c->N * sizeof(float)); if (rc) return rc; }
+    if (!c->d_dat) { int rc = dev_alloc(c, (void**)&c->d_dat, (size_t)c->prm.nt * (size_t)std::max(c->L, 1) * sizeof(float)); if (rc) return rc; }
+    return PACT_OK;
+}
+
+extern "C" int pact_forward_host(pact_ctx* c, const float* p0_host, float* data_host)
+{
+    if (!c || !p0_host || (!data_host && c->L > 0)) return PACT_EINVAL;
+    int rc = ensure_host_staging(c);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(c->d_vol, p0_host, (size_t)c->N * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    if ((rc = pact_forward(c, c->d_vol, c->d_dat))) return rc;
+    if (c->L > 0)
+        CK(cudaMemcpyAsync(data_host, c->d_dat, (size_t)c->prm.nt * c->L * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    return PACT_OK;
+}
+
+extern "C" int pact_adjoint_host(pact_ctx* c, const float* data_host, float* image_host)
+{
+    if (!c || !image_host || (!data_host && c->L > 0)) return PACT_EINVAL;
+    int rc = ensure_host_staging(c);
+    if (rc) return rc;
+    if (c->L > 0)
+        CK(cudaMemcpyAsync(c->d_dat, data_host, (size_t)c->prm.nt * c->L * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    if ((rc = pact_adjoint(c, c->d_dat, c->d_vol))) return rc;
+    CK(cudaMemcpyAsync(image_host, c->d_vol, (size_t)c->N * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    return PACT_OK;
+}
+
+// ---- options and timing -------------------------------------------------------------------------
+extern "C" int pact_set_option(pact_ctx* c, const char* key, long long value)
+{
+    if (!c || !key) return PACT_EINVAL;
+    if (!strcmp(key, "profile")) { c->profile = value != 0; return PACT_OK; }
+    if (!strcmp(key, "variant")) {
+        if (value < 0 || value > 2) return PACT_EINVAL;
+        c->variant = (int)value;
+        return PACT_OK;
+    }
+    if (!strcmp(key, "graph")) { c->use_graph = value < 0 ? -1 : (value != 0); return PACT_OK; }
+    return PACT_EINVAL;
+}
+
+extern "C" int pact_get_timing(pact_ctx* c, int op, double* loop_ms, double* kernel_ms, long long* launches)
+{
+    if (!c || op < 0 || op > 1 || !c->have_timing[op]) return PACT_EINVAL;
+    CK(cudaStreamSynchronize(c->stream));
+    if (loop_ms) {
+        float ms = 0.0f;
+        CK(cudaEventElapsedTime(&ms, c->ev_loop[op][0], c->ev_loop[op][1]));
+        *loop_ms = ms;
+    }
+    for (int k = 0; k < 8; ++k) {
+        if (kernel_ms) {
+            double acc = 0.0;
+            for (size_t s = 0; s < c->used[op][k]; ++s) {
+                float ms = 0.0f;
+                CK(cudaEventElapsedTime(&ms, c->samples[op][k][s].a, c->samples[op][k][s].b));
+                acc += ms;
+            }
+            kernel_ms[k] = c->used[op][k] ? acc / (double)c->used[op][k] : 0.0;
+        }
+        if (launches) launches[k] = c->launches[op][k];
+    }
+    return PACT_OK;
+}

@@ -395,3 +395,19 @@ def custom_problem(name, prm: Params, cp, cs, rho, alpha, rcv, p0) -> Problem:
 def gaussian_ball(prm: Params, c, sigma, amp=1.0, cut=3.5) -> np.ndarray:
     """amp*exp(-r^2/(2 sigma^2)) on the nodes, zero beyond cut*sigma (float64 volume)."""
     return _gaussian_blob(prm, np.asarray(c, dtype=np.float64), sigma, amp, cut)
+
+
+def crop(prob: Problem, origin, n, nt: int) -> Problem:
+    """Sub-block [z0:z0+n, y0:y0+n, x0:x0+n] of a problem's volumes with the receivers that fall
+    inside it (shifted to the block's origin) and `nt` samples — a bounded sample of the same
+    workload for timing the CPU oracle (bench.py `cpu_baseline`, `--impl reference`)."""
+    from dataclasses import replace
+    x0, y0, z0 = (int(v) for v in origin)
+    sl = (slice(z0, z0 + n), slice(y0, y0 + n), slice(x0, x0 + n))
+    prm = replace(prob.prm, nx=n, ny=n, nz=n, nt=nt)
+    r = prob.rcv - np.array([x0, y0, z0], dtype=np.float64) * prob.prm.h
+    keep = np.all((r >= 0.0) & (r <= (n - 1) * prob.prm.h), axis=1)
+    cut = lambda a: None if a is None else np.ascontiguousarray(a[sl])
+    return Problem(name=f"{prob.name}-crop{n}", prm=prm, lam=cut(prob.lam), mu=cut(prob.mu), rho=cut(prob.rho),
+                   alpha=cut(prob.alpha), rcv=np.ascontiguousarray(r[keep]), p0=cut(prob.p0),
+                   meta=dict(origin=(x0, y0, z0), parent=prob.name))

@@ -1,0 +1,193 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 CPU oracle, element by element,
+on the same seeded inputs.  Tolerances are north_star's: relative L2 <= 1e-4 on receiver data and
+images, adjoint dot-product test <= 1e-5 (fp32 path; inner products accumulated in fp64)."""
+import numpy as np
+import pytest
+
+from paper_1709_02733_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+TOL_L2 = 1e-4     # north_star: GPU (fp32) vs oracle (fp64), relative L2
+TOL_DOT = 1e-5    # north_star: adjoint dot-product test of the fp32 path
+
+
+def rel_l2(a, b):
+    a = np.asarray(a, dtype=np.float64)
+    b = np.asarray(b, dtype=np.float64)
+    return float(np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300))
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "the gpu-marked tests need a CUDA device"
+    from paper_1709_02733_b200 import build
+    build.build()
+    return torch
+
+
+def gpu_ops(torch, prob, variant=0, graph=-1):
+    from paper_1709_02733_b200.binding import Pact
+    ctx = Pact.from_problem(prob)
+    ctx.set_option("variant", variant)
+    ctx.set_option("graph", graph)
+    return ctx
+
+
+def run_pair(torch, prob, x, y, variant=0, graph=-1):
+    ctx = gpu_ops(torch, prob, variant, graph)
+    xd = torch.from_numpy(np.ascontiguousarray(x, dtype=np.float32)).cuda()
+    yd = torch.from_numpy(np.ascontiguousarray(y, dtype=np.float32)).cuda()
+    Hx = ctx.forward(xd).cpu().numpy()
+    Hty = ctx.adjoint(yd).cpu().numpy()
+    ctx.close()
+    return Hx, Hty
+
+
+def oracle_pair(prob, x, y):
+    from oracle.oracle import Oracle
+    o = Oracle.from_problem(prob)
+    x32 = np.asarray(x, dtype=np.float32).astype(np.float64)   # both sides see the same fp32 inputs
+    y32 = np.asarray(y, dtype=np.float32).astype(np.float64)
+    Hx, Hty = o.forward(x32), o.adjoint(y32)
+    o.close()
+    return Hx, Hty
+
+
+VARIANTS = [1]
+
+# sizes span several 32x8x2 / 64x16 tiles plus ragged tails in every axis
+RANDOM_CASES = [
+    dict(nx=45, ny=37, nz=41, nt=40, npml=5, L=19, seed=1, lossy=True),
+    dict(nx=70, ny=34, nz=29, nt=30, npml=4, L=11, seed=2, lossy=True),
+    dict(nx=33, ny=66, nz=20, nt=25, npml=0, L=9, seed=3, lossy=False),
+    dict(nx=8, ny=8, nz=8, nt=12, npml=0, L=3, seed=4, lossy=True),          # minimum grid
+    dict(nx=16, ny=17, nz=18, nt=20, npml=4, L=5, seed=5, lossy=True),       # 2*npml+8 == nx: thickest legal PML
+]
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("case", RANDOM_CASES, ids=lambda c: f"{c['nx']}x{c['ny']}x{c['nz']}_p{c['npml']}")
+def test_random_heterogeneous_parity_and_dot(torch_cuda, case, variant):
+    """Random heterogeneous solid/fluid medium (40 % fluid cells), off-node receivers, random x, y."""
+    prob = synth.random_problem(**case)
+    x, y = synth.random_vectors(prob, seed=case["seed"])
+    Hx, Hty = run_pair(torch_cuda, prob, x, y, variant)
+    Hx_o, Hty_o = oracle_pair(prob, x, y)
+    assert rel_l2(Hx, Hx_o) <= TOL_L2
+    assert rel_l2(Hty, Hty_o) <= TOL_L2
+    x32, y32 = x.astype(np.float32).astype(np.float64), y.astype(np.float32).astype(np.float64)
+    a, b = np.vdot(Hx.astype(np.float64), y32), np.vdot(x32, Hty.astype(np.float64))
+    assert abs(a - b) <= TOL_DOT * max(abs(a), abs(b))
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_config1_full(torch_cuda, variant):
+    """BASELINE config 1 at full size (64^3, 300 samples, 128 receivers): forward, adjoint, dot test."""
+    prob = synth.make_config(1)
+    Hx_o, _ = oracle_pair(prob, prob.p0, np.zeros((prob.prm.nt, prob.L)))
+    rng = np.random.default_rng(11)
+    y = Hx_o + 0.05 * np.abs(Hx_o).max() * rng.standard_normal(Hx_o.shape)
+    Hx, Hty = run_pair(torch_cuda, prob, prob.p0, y, variant)
+    _, Hty_o = oracle_pair(prob, np.zeros(prob.p0.shape), y)
+    assert rel_l2(Hx, Hx_o) <= TOL_L2
+    assert rel_l2(Hty, Hty_o) <= TOL_L2
+    y32 = y.astype(np.float32).astype(np.float64)
+    a, b = np.vdot(Hx.astype(np.float64), y32), np.vdot(prob.p0.astype(np.float64), Hty.astype(np.float64))
+    assert abs(a - b) <= TOL_DOT * max(abs(a), abs(b))
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_config2_truncated(torch_cuda, variant):
+    """BASELINE config 2 (128^3 skull shell, absorption in the shell) on its real volumes, 160 samples."""
+    prob = synth.make_config(2, nt=160)
+    rng = np.random.default_rng(12)
+    y = rng.standard_normal((prob.prm.nt, prob.L))
+    Hx, Hty = run_pair(torch_cuda, prob, prob.p0, y, variant)
+    Hx_o, Hty_o = oracle_pair(prob, prob.p0, y)
+    assert rel_l2(Hx, Hx_o) <= TOL_L2
+    assert rel_l2(Hty, Hty_o) <= TOL_L2
+
+
+def test_graph_and_direct_launch_agree_bitwise(torch_cuda):
+    prob = synth.random_problem(nx=40, ny=24, nz=33, nt=30, npml=4, L=7, seed=6)
+    x, y = synth.random_vectors(prob, seed=6)
+    a = run_pair(torch_cuda, prob, x, y, graph=1)
+    b = run_pair(torch_cuda, prob, x, y, graph=0)
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+
+
+def test_calls_are_repeatable_and_independent(torch_cuda):
+    """Each call resets the state: forward, adjoint, forward again gives bit-identical data."""
+    torch = torch_cuda
+    prob = synth.random_problem(nx=24, ny=20, nz=28, nt=20, npml=4, L=6, seed=7)
+    x, y = synth.random_vectors(prob, seed=7)
+    ctx = gpu_ops(torch, prob)
+    xd, yd = torch.from_numpy(x.astype(np.float32)).cuda(), torch.from_numpy(y.astype(np.float32)).cuda()
+    d1 = ctx.forward(xd).clone()
+    i1 = ctx.adjoint(yd).clone()
+    d2 = ctx.forward(xd)
+    i2 = ctx.adjoint(yd)
+    assert torch.equal(d1, d2) and torch.equal(i1, i2)
+    ctx.close()
+
+
+def test_host_buffer_entry_points(torch_cuda):
+    torch = torch_cuda
+    prob = synth.random_problem(nx=24, ny=20, nz=28, nt=20, npml=4, L=6, seed=8)
+    x, y = synth.random_vectors(prob, seed=8)
+    ctx = gpu_ops(torch, prob)
+    xh = torch.from_numpy(x.astype(np.float32)).pin_memory()
+    yh = torch.from_numpy(y.astype(np.float32)).pin_memory()
+    dh = torch.empty((prob.prm.nt, prob.L), dtype=torch.float32).pin_memory()
+    ih = torch.empty(prob.p0.shape, dtype=torch.float32).pin_memory()
+    ctx.forward_host(xh, dh)
+    ctx.adjoint_host(yh, ih)
+    assert torch.equal(dh, ctx.forward(xh.cuda()).cpu())
+    assert torch.equal(ih, ctx.adjoint(yh.cuda()).cpu())
+    ctx.close()
+
+
+def test_error_codes(torch_cuda):
+    torch = torch_cuda
+    from dataclasses import replace
+    from paper_1709_02733_b200.binding import Pact, PactError
+    prob = synth.random_problem(nx=16, ny=16, nz=16, nt=5, npml=2, L=3, seed=9)
+    with pytest.raises(PactError) as e:   # dt above the stability limit
+        Pact.from_problem(replace(prob, prm=replace(prob.prm, dt=prob.prm.dt * 3.0)))
+    assert e.value.code == -2
+    bad = prob.rcv.copy(); bad[0, 0] = -prob.prm.h
+    with pytest.raises(PactError) as e:   # receiver outside the grid
+        Pact.from_problem(replace(prob, rcv=bad))
+    assert e.value.code == -3
+    rho = prob.rho.copy(); rho[3, 4, 5] = 0.0
+    with pytest.raises(PactError) as e:   # rho <= 0
+        Pact.from_problem(replace(prob, rho=rho))
+    assert e.value.code == -4
+    lam = prob.lam.copy(); lam[0, 0, 0] = np.nan
+    with pytest.raises(PactError) as e:
+        Pact.from_problem(replace(prob, lam=lam))
+    assert e.value.code == -4
+    with pytest.raises(PactError) as e:   # PML too thick for the grid
+        Pact.from_problem(replace(prob, prm=replace(prob.prm, npml=5)))
+    assert e.value.code == -1
+
+
+def test_no_receivers_and_lossless_null_alpha(torch_cuda):
+    """L = 0 is legal (data is empty, image is zero); alpha = NULL means lossless."""
+    torch = torch_cuda
+    from dataclasses import replace
+    from paper_1709_02733_b200.binding import Pact
+    prob = synth.random_problem(nx=20, ny=18, nz=16, nt=15, npml=3, L=4, seed=10, lossy=False)
+    x, y = synth.random_vectors(prob, seed=10)
+    a = Pact.from_problem(prob)
+    b = Pact.from_problem(replace(prob, alpha=None))
+    xd = torch.from_numpy(x.astype(np.float32)).cuda()
+    assert torch.equal(a.forward(xd), b.forward(xd))
+    c = Pact.from_problem(replace(prob, rcv=np.zeros((0, 3))))
+    assert c.forward(xd).shape == (prob.prm.nt, 0)
+    img = c.adjoint(torch.empty((prob.prm.nt, 0), dtype=torch.float32, device="cuda"))
+    assert float(img.abs().max()) == 0.0
+    for k in (a, b, c):
+        k.close()
