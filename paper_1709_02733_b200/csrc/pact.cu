@@ -42,6 +42,7 @@ struct EvPair { cudaEvent_t a, b; };
 struct pact_ctx {
     pact_params prm;
     cudaStream_t stream;
+    cudaStream_t cap_stream;   // private stream for graph capture (the legacy default stream cannot capture)
     long long N;             // nx ny nz
     int L;
     int pitch, py, pz;       // padded box extents
@@ -126,6 +127,7 @@ extern "C" void pact_destroy(pact_ctx* c)
     if (!c) return;
     cudaStreamSynchronize(c->stream);
     free_graphs(c);
+    if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     for (int op = 0; op < 2; ++op) {
         for (int k = 0; k < 8; ++k)
             for (auto& s : c->samples[op][k]) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
@@ -451,9 +453,13 @@ static int run_loop(pact_ctx* c, int which /*0 fwd, 1 adj*/)
         }
         if (!c->gexec[which]) {
             cudaGraph_t graph = nullptr;
-            CK(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+            if (!c->cap_stream) CK(cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking));
+            cudaStream_t user = c->stream;
+            CK(cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal));
+            c->stream = c->cap_stream;
             int rc = which == 0 ? enqueue_forward_loop(c, false, variant) : enqueue_adjoint_loop(c, false, variant);
-            cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+            c->stream = user;
+            cudaError_t e = cudaStreamEndCapture(c->cap_stream, &graph);
             if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
             if (e != cudaSuccess) return cuda_fail(e, "cudaStreamEndCapture", __LINE__);
             e = cudaGraphInstantiate(&c->gexec[which], graph, 0);
