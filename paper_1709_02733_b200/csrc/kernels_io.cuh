@@ -136,3 +136,32 @@ __global__ void k_scatter(const DevGrid g, const RcvTables r, const IoArgs* __re
     const long long n = r.tnode[k];
     g.f[S11][n] -= acc; g.f[S22][n] -= acc; g.f[S33][n] -= acc;
 }
+
+// ---- scaled adjoint variables of the fused variant --------------------
+// The fused adjoint carries s = C sigma_bar (C = the dt/h-scaled isotropic stiffness of Eq. 7c).  For a
+// source that adds the same value v to the three normal components, C (v,v,v) = (3 Ll + 2 Ml) (v,v,v).
+__device__ __forceinline__ float bulk3(const DevGrid& g, long long n) { return 3.0f * g.Ll[n] + 2.0f / g.Mi[n]; }
+
+__global__ void k_scatter_scaled(const DevGrid g, const RcvTables r, const IoArgs* __restrict__ io, int m)
+{
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= r.nnodes) return;
+    const float* __restrict__ d = io->data_in + (long long)m * r.L;
+    float acc = 0.0f;
+    for (int e = r.row_ptr[k]; e < r.row_ptr[k + 1]; ++e) acc = fmaf(r.tw[e], d[r.trcv[e]], acc);
+    const long long n = r.tnode[k];
+    acc *= bulk3(g, n);
+    g.f[S11][n] -= acc; g.f[S22][n] -= acc; g.f[S33][n] -= acc;
+}
+
+// tau^T on the scaled variables: sigma_bar11+22+33 = (s11+s22+s33) / (3 Ll + 2 Ml)
+__global__ void k_image_scaled(const DevGrid g, const IoArgs* __restrict__ io)
+{
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int y = blockIdx.y * blockDim.y + threadIdx.y;
+    const int z = blockIdx.z;
+    if (x >= g.nx || y >= g.ny) return;
+    const long long i = (long long)z * g.sz + (long long)y * g.sy + x;
+    io->image[(long long)x + (long long)g.nx * ((long long)y + (long long)g.ny * z)] =
+        (g.f[S11][i] + g.f[S22][i] + g.f[S33][i]) / bulk3(g, i) * (-1.0f / 3.0f);
+}

@@ -19,7 +19,9 @@
 #include "common.cuh"
 #include "kernels_io.cuh"
 #include "kernels_plain.cuh"
-#include "kernels_tiled.cuh"
+#include "kernels_fused.cuh"
+
+#define PACT_DEFAULT_VARIANT 1
 
 // ------------------------------------------------------------------------------------------------
 static thread_local char g_cuda_err[512] = "";
@@ -56,6 +58,15 @@ struct pact_ctx {
     float* state_base;
     long long state_bytes;
     float* scratch_base;     // adjoint scratch of the plain variant, allocated on first use
+    // fused variant (kernels_fused.cuh): second state buffer, ping-pong memory variables, TMA maps
+    bool fused_ready;
+    DevGrid g2;              // view of state buffer B for the I/O kernels
+    float* stateB_base;
+    long long stateB_bytes;
+    CUtensorMap tmS40[2], tmS36[2], tmM40, tmM36;
+    FusedArgs fa;
+    int zchunk;              // planes per CTA along z (0 = auto)
+    float* mvbuf[2][18];     // fused memory variables, two sets (read / written alternate every step)
     // host-buffer variants
     float* d_vol;            // [N]
     float* d_dat;            // [nt][L]
@@ -371,10 +382,6 @@ static void forward_step(pact_ctx* c, Launcher& ln, int variant)
 {
     const DevGrid& g = c->g;
     cudaStream_t st = c->stream;
-    if (variant == 2) {
-        tiled_forward_step(g, st, ln);
-        return;
-    }
     dim3 blk(PLAIN_BX, PLAIN_BY, PLAIN_BZ);
     dim3 grd((g.nx + PLAIN_BX - 1) / PLAIN_BX, (g.ny + PLAIN_BY - 1) / PLAIN_BY, (g.nz + PLAIN_BZ - 1) / PLAIN_BZ);
     ln.run(PACT_K_FWD_VEL, [&] { k_fwd_vel<<<grd, blk, 0, st>>>(g); });
@@ -385,16 +392,126 @@ static void adjoint_step(pact_ctx* c, Launcher& ln, int variant)
 {
     const DevGrid& g = c->g;
     cudaStream_t st = c->stream;
-    if (variant == 2) {
-        tiled_adjoint_step(g, st, ln);
-        return;
-    }
     dim3 blk(PLAIN_BX, PLAIN_BY, PLAIN_BZ);
     dim3 grd((g.nx + PLAIN_BX - 1) / PLAIN_BX, (g.ny + PLAIN_BY - 1) / PLAIN_BY, (g.nz + PLAIN_BZ - 1) / PLAIN_BZ);
     ln.run(PACT_K_ADJ_A, [&] { k_adj_a1<<<grd, blk, 0, st>>>(g); });
     ln.run(PACT_K_ADJ_A, [&] { k_adj_a2<<<grd, blk, 0, st>>>(g); });
     ln.run(PACT_K_ADJ_B, [&] { k_adj_b1<<<grd, blk, 0, st>>>(g); });
     ln.run(PACT_K_ADJ_B, [&] { k_adj_b2<<<grd, blk, 0, st>>>(g); });
+}
+
+
+// ---- fused variant: buffers, TMA descriptors, launch ---------------------------------------------
+typedef CUresult (*encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// 4-D map [field][z][y][x] over `nf` padded fields starting at `base` (start of the padded box), box {bw, bh, 1, 1}
+static int make_map(pact_ctx* c, encode_tiled_fn enc, CUtensorMap* tm, const float* base, int nf, int bw, int bh)
+{
+    const cuuint64_t dims[4] = {(cuuint64_t)c->pitch, (cuuint64_t)c->py, (cuuint64_t)c->pz, (cuuint64_t)nf};
+    const cuuint64_t strides[3] = {(cuuint64_t)c->pitch * 4, (cuuint64_t)c->pitch * c->py * 4, (cuuint64_t)c->box * 4};
+    const cuuint32_t boxd[4] = {(cuuint32_t)bw, (cuuint32_t)bh, 1, 1};
+    const cuuint32_t es[4] = {1, 1, 1, 1};
+    CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (void*)base, dims, strides, boxd, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                     CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+        return PACT_ECUDA;
+    }
+    return PACT_OK;
+}
+
+static int ensure_fused(pact_ctx* c)
+{
+    if (c->fused_ready) return PACT_OK;
+    const DevGrid& g = c->g;
+    const int P = g.P;
+    FusedArgs& fa = c->fa;
+    memset(&fa, 0, sizeof(fa));
+    fa.nx = g.nx; fa.ny = g.ny; fa.nz = g.nz;
+    fa.ntx = (g.nx + FT_TX - 1) / FT_TX; fa.nty = (g.ny + FT_TY - 1) / FT_TY;
+    fa.sy = g.sy; fa.sz = g.sz; fa.box = c->box;
+    fa.P = P;
+    fa.nxq = (g.nx + 3) / 4 * 4;
+    fa.wyz = P > 0 ? 2 * P + 1 : 0;
+    if (P > 0) {
+        fa.xl = (P + 3) / 4 * 4;
+        fa.xr = (g.nx - 1 - P) / 4 * 4;
+        if (fa.xl >= fa.xr) { fa.xl = fa.nxq; fa.xr = fa.nxq; }
+        fa.wx = fa.xl + (fa.nxq - fa.xr);
+    }
+    for (int b = 0; b < 3; ++b)
+        for (int t = 0; t < 4; ++t) fa.tab[b][t] = g.tab[b][t];
+    // state buffer B + ping-pong memory variables in one block (zeroed at the start of every call)
+    long long mv[3] = {0, 0, 0};
+    if (P > 0) {
+        mv[0] = (long long)fa.wx * g.ny * g.nz;
+        mv[1] = (long long)fa.nxq * fa.wyz * g.nz;
+        mv[2] = (long long)fa.nxq * g.ny * fa.wyz;
+    }
+    auto r32 = [](long long v) { return (v + 31) / 32 * 32; };
+    long long total = c->box * NFIELD;
+    for (int b = 0; b < 3; ++b) total += 2 * 6 * r32(mv[b]);
+    c->stateB_bytes = total * (long long)sizeof(float);
+    int rc = dev_alloc(c, (void**)&c->stateB_base, (size_t)c->stateB_bytes);
+    if (rc) return rc;
+    const long long org = (long long)PACT_HALO_Z * g.sz + (long long)PACT_HALO_Y * g.sy + PACT_HALO_X;
+    c->g2 = c->g;
+    for (int k = 0; k < NFIELD; ++k) c->g2.f[k] = c->stateB_base + (long long)k * c->box + org;
+    {
+        float* p = c->stateB_base + c->box * NFIELD;
+        for (int set = 0; set < 2; ++set)            // [0]: read at even steps, [1]: read at odd steps
+            for (int k = 0; k < 18; ++k) { c->mvbuf[set][k] = p; p += r32(mv[k % 3]); }
+    }
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    CK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+    if (!fn || qres != cudaDriverEntryPointSuccess) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "cuTensorMapEncodeTiled is not available from the driver");
+        return PACT_ECUDA;
+    }
+    encode_tiled_fn enc = (encode_tiled_fn)fn;
+    const float* baseA = c->state_base;
+    const float* baseB = c->stateB_base;
+    const float* baseM = g.Ll - org;
+    if ((rc = make_map(c, enc, &c->tmS40[0], baseA, NFIELD, FT_BW, FT_BH))) return rc;
+    if ((rc = make_map(c, enc, &c->tmS36[0], baseA, NFIELD, FT_BW, FT_UH))) return rc;
+    if ((rc = make_map(c, enc, &c->tmS40[1], baseB, NFIELD, FT_BW, FT_BH))) return rc;
+    if ((rc = make_map(c, enc, &c->tmS36[1], baseB, NFIELD, FT_BW, FT_UH))) return rc;
+    if ((rc = make_map(c, enc, &c->tmM40, baseM, 4, FT_BW, FT_BH))) return rc;
+    if ((rc = make_map(c, enc, &c->tmM36, baseM, 4, FT_MW, FT_MH))) return rc;
+    CK(cudaFuncSetAttribute(k_fused<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
+    CK(cudaFuncSetAttribute(k_fused<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
+    fa.mat = g.Ll;
+    c->fused_ready = true;
+    return PACT_OK;
+}
+
+// one time step cur -> 1-cur ; sgn = +1: W' ; sgn = -1: W'^T on the scaled adjoint variables
+static void fused_step(pact_ctx* c, Launcher& ln, int cur, float sgn, int kind)
+{
+    FusedArgs fa = c->fa;
+    const DevGrid& gi = cur ? c->g2 : c->g;
+    const DevGrid& go = cur ? c->g : c->g2;
+    fa.in = gi.f[0]; fa.out = go.f[0];
+    fa.sgn = sgn;
+    for (int k = 0; k < 18; ++k) { fa.mvi[k] = c->mvbuf[cur][k]; fa.mvo[k] = c->mvbuf[1 - cur][k]; }
+    int zc = c->zchunk;
+    if (zc <= 0) {
+        // enough CTAs for ~7 waves of 148 SMs, chunks no shorter than 32 planes
+        const int tiles = fa.ntx * fa.nty;
+        int nzc = std::max(1, (7 * 148 + tiles - 1) / tiles);
+        zc = std::max(32, (fa.nz + nzc - 1) / nzc);
+    }
+    zc = std::min(zc, fa.nz);
+    fa.zc = zc; fa.nzc = (fa.nz + zc - 1) / zc;
+    const int grid = fa.ntx * fa.nty * fa.nzc;
+    cudaStream_t st = c->stream;
+    if (fa.P > 0)
+        ln.run(kind, [&] { k_fused<true><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM40, c->tmM36, fa); });
+    else
+        ln.run(kind, [&] { k_fused<false><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM40, c->tmM36, fa); });
 }
 
 // Eq. 58 right to left: tau, then for m = 0..M-1 { Theta ; W' unless m = M-1 }
@@ -406,10 +523,15 @@ static int enqueue_forward_loop(pact_ctx* c, bool profile, int variant)
     Launcher ln{c, 0, false, 0};
     const int every = std::max(1, (nt - 1) / MAX_SAMPLES);
     const dim3 rblk(128), rgrd((c->L + 127) / 128);
+    int cur = 0;   // fused variant: which state buffer holds v'_m
     for (int m = 0; m < nt; ++m) {
         ln.sample = profile && (m % every == every / 2);
-        if (c->L > 0) ln.run(PACT_K_RECV, [&] { k_gather<<<rgrd, rblk, 0, st>>>(g, c->rcv, c->d_io, m); });
-        if (m < nt - 1) forward_step(c, ln, variant);
+        const DevGrid& gc = cur ? c->g2 : g;
+        if (c->L > 0) ln.run(PACT_K_RECV, [&] { k_gather<<<rgrd, rblk, 0, st>>>(gc, c->rcv, c->d_io, m); });
+        if (m < nt - 1) {
+            if (variant == 2) { fused_step(c, ln, cur, 1.0f, PACT_K_FWD_FUSED); cur ^= 1; }
+            else forward_step(c, ln, variant);
+        }
     }
     return ln.err;
 }
@@ -424,10 +546,25 @@ static int enqueue_adjoint_loop(pact_ctx* c, bool profile, int variant)
     Launcher ln{c, 1, false, 0};
     const int every = std::max(1, (nt - 1) / MAX_SAMPLES);
     const dim3 rblk(128), rgrd((c->rcv.nnodes + 127) / 128);
+    int cur = 0;
     for (int m = nt - 1; m >= 0; --m) {
         ln.sample = profile && (m % every == every / 2);
-        if (m < nt - 1) adjoint_step(c, ln, variant);
-        if (c->L > 0) ln.run(PACT_K_RECV, [&] { k_scatter<<<rgrd, rblk, 0, st>>>(g, c->rcv, c->d_io, m); });
+        if (m < nt - 1) {
+            if (variant == 2) { fused_step(c, ln, cur, -1.0f, PACT_K_ADJ_FUSED); cur ^= 1; }
+            else adjoint_step(c, ln, variant);
+        }
+        const DevGrid& gc = cur ? c->g2 : g;
+        if (c->L > 0) {
+            if (variant == 2) ln.run(PACT_K_RECV, [&] { k_scatter_scaled<<<rgrd, rblk, 0, st>>>(gc, c->rcv, c->d_io, m); });
+            else ln.run(PACT_K_RECV, [&] { k_scatter<<<rgrd, rblk, 0, st>>>(gc, c->rcv, c->d_io, m); });
+        }
+    }
+    ln.sample = false;
+    {   // tau^T (Eq. 27c / 60c)
+        const DevGrid& gc = cur ? c->g2 : g;
+        dim3 blk(64, 4), grd((g.nx + 63) / 64, (g.ny + 3) / 4, g.nz);
+        if (variant == 2) ln.run(PACT_K_OTHER, [&] { k_image_scaled<<<grd, blk, 0, st>>>(gc, c->d_io); });
+        else ln.run(PACT_K_OTHER, [&] { k_image<<<grd, blk, 0, st>>>(gc, c->d_io); });
     }
     return ln.err;
 }
@@ -444,6 +581,11 @@ static int run_loop(pact_ctx* c, int which /*0 fwd, 1 adj*/)
 {
     const int variant = resolve_variant(c);
     if (which == 1 && variant == 1) { int rc = ensure_scratch(c); if (rc) return rc; }
+    if (variant == 2) {
+        int rc = ensure_fused(c);
+        if (rc) return rc;
+        CK(cudaMemsetAsync(c->stateB_base, 0, (size_t)c->stateB_bytes, c->stream));
+    }
     for (int k = 0; k < 8; ++k) { c->used[which][k] = 0; c->launches[which][k] = 0; }
     c->have_timing[which] = c->profile != 0;
     if (want_graph(c)) {
@@ -497,12 +639,7 @@ extern "C" int pact_adjoint(pact_ctx* c, const float* data, float* image)
     IoArgs io{nullptr, nullptr, data, image};
     k_set_io<<<1, 1, 0, st>>>(c->d_io, io);
     CK(cudaMemsetAsync(c->state_base, 0, (size_t)c->state_bytes, st));
-    int rc = run_loop(c, 1);
-    if (rc) return rc;
-    dim3 blk(64, 4), grd((c->g.nx + 63) / 64, (c->g.ny + 3) / 4, c->g.nz);
-    k_image<<<grd, blk, 0, st>>>(c->g, c->d_io);
-    CK(cudaGetLastError());
-    return PACT_OK;
+    return run_loop(c, 1);
 }
 
 // ---- host-buffer variants -----------------------------------------------------------------------
@@ -549,6 +686,7 @@ extern "C" int pact_set_option(pact_ctx* c, const char* key, long long value)
         c->variant = (int)value;
         return PACT_OK;
     }
+    if (!strcmp(key, "zchunk")) { if (value < 0) return PACT_EINVAL; c->zchunk = (int)value; free_graphs(c); return PACT_OK; }
     if (!strcmp(key, "graph")) { c->use_graph = value < 0 ? -1 : (value != 0); return PACT_OK; }
     return PACT_EINVAL;
 }
