@@ -108,7 +108,10 @@ const char* pact_last_cuda_error(void);
  *              pact_get_timing.  0 (default): no events.
  *   "variant"  step-kernel implementation: 0 = default (best available), 1 = plain two-kernel
  *              in-place path, 2 = fused single-pass path.
- *   "graph"    1: replay the time loop from a captured CUDA graph (default for small grids).
+ *   "graph"    1: replay the time loop from a captured CUDA graph (default for small grids);
+ *              0: launch directly; -1: automatic.
+ *   "zchunk"   planes of z each CTA of the fused kernel marches over (0 = automatic).  Any value
+ *              gives the same operator; it only changes how the grid is cut into CTAs.
  */
 int pact_set_option(pact_ctx* ctx, const char* key, long long value);
 

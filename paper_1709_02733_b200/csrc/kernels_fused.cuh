@@ -10,11 +10,21 @@
 //   stage 1 (Eq. 46a,b): u(kk) on the tile + 2 cells of ring, from sigma on the tile + 4 cells;
 //   stage 2 (Eq. 46c,d): sigma(kk-2) on the tile, from u(kk-4 .. kk) kept in a shared-memory ring.
 // Fields whose x/y neighbours are needed (s11,s22,s12,s13,s23, rho, alpha, mu) and s33 arrive in
-// shared memory by TMA (cp.async.bulk.tensor, mbarrier complete_tx), one plane ahead of use; the
+// shared memory by TMA (cp.async.bulk.tensor, mbarrier complete_tx), two planes ahead of use; the
 // z neighbours of s13,s23,s33 live in per-thread register windows; u_old, lambda and the old
 // s11,s22,s12 are own-column values fetched with 128-bit loads one stage ahead of use.
 // The ring of 2 (4) cells around the tile is recomputed by the neighbouring CTAs; nothing is
 // exchanged between CTAs, hence the two state buffers.
+//
+// Synchronisation: ONE __syncthreads per plane (between the stages).  The z taps of stage 2 are
+// own-column reads of the u ring, so the only cross-thread reads of a ring slot happen while it is
+// the centre plane; TMA refills are issued by thread 0 right after the barrier into slots whose
+// last readers finished before it (slot algebra in DESIGN.md "Fused kernel").
+//
+// C-PML (Eq. 46a,c / 61): memory variables are slab-confined, read from one set and written to the
+// other (the tile ring recomputes them without writing).  Forward: the recursion follows the
+// difference (own quad only).  Adjoint: the recursion precedes the difference, so the taps of the
+// difference along the slab axis are re-derived from the neighbours' old memory variables.
 #pragma once
 #include <cuda.h>
 #include "common.cuh"
@@ -46,6 +56,11 @@
 #define FT_OFF_END (FT_OFF_UR + 3 * FT_RING * FT_UPL)
 #define FT_SMEM_BYTES (FT_OFF_END * 4 + 64)   // + 8 mbarriers
 
+// kernel modes: which C-PML code a launch carries (CTAs away from the slabs skip it at run time)
+#define FM_PLAIN 0     // no C-PML (npml = 0)
+#define FM_FWD 1       // W'   : Eq. 46a-d, memory variables updated after differencing
+#define FM_ADJ 2       // W'^T : Eq. 61, memory variables (tilde form) applied before differencing
+
 struct FusedArgs {
     int nx, ny, nz;
     int ntx, nty;          // tiles along x, y
@@ -56,7 +71,7 @@ struct FusedArgs {
     float* out;            // state written
     const float* mat;      // scaled materials Ll, Mi, Rr, Aa at mat + k*box (node (0,0,0))
     float sgn;             // +1: W' on (u, sigma) ; -1: W'^T on the scaled adjoint variables
-    // C-PML (PML variant only)
+    // C-PML
     int P;
     const float* tab[3][4];
     int xl, xr, wx;        // x slab: columns [0,xl) and [xr, nxq) ; wx = xl + nxq - xr ; quad aligned
@@ -109,27 +124,38 @@ __device__ __forceinline__ float4 fma4(float4 a, float4 b, float4 c)
 {
     return make_float4(fmaf(a.x, b.x, c.x), fmaf(a.y, b.y, c.y), fmaf(a.z, b.z, c.z), fmaf(a.w, b.w, c.w));
 }
+__device__ __forceinline__ float4 fma4(float a, float4 b, float4 c)
+{
+    return make_float4(fmaf(a, b.x, c.x), fmaf(a, b.y, c.y), fmaf(a, b.z, c.z), fmaf(a, b.w, c.w));
+}
 // the value one x to the right of each lane of `c`, `r0` being the element after c.w
 __device__ __forceinline__ float4 shl1(float4 c, float r0) { return make_float4(c.y, c.z, c.w, r0); }
-__device__ __forceinline__ float4 rcp4(float4 a) { return make_float4(__frcp_rn(a.x), __frcp_rn(a.y), __frcp_rn(a.z), __frcp_rn(a.w)); }
+// 1/x by the special-function unit (MUFU.RCP, <= 1 ulp): 1/inf = 0 (fluid: mu = 0), 1/0 = inf
+__device__ __forceinline__ float rcpa(float x)
+{
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float4 rcp4(float4 a) { return make_float4(rcpa(a.x), rcpa(a.y), rcpa(a.z), rcpa(a.w)); }
 
-// Eq. 8 without 1/h, along y or z: taps t0..t3 at consecutive samples;
-//   D+ at i uses (i-1, i, i+1, i+2) ; D- at i uses (i-2, i-1, i, i+1)
+// Eq. 8 without 1/h and divided by c2 = -1/24 (both folded into the scaled
+// coefficients):  (9/8 (t2 - t1) - 1/24 (t3 - t0)) / c2 = (t3 - t0) - 27 (t2 - t1).
+// Taps t0..t3 at consecutive samples: D+ at i uses (i-1, i, i+1, i+2) ; D- at i uses (i-2, i-1, i, i+1).
+#define FT_K 27.0f
+__device__ __forceinline__ float d1(float t0, float t1, float t2, float t3) { return fmaf(-FT_K, t2 - t1, t3 - t0); }
 __device__ __forceinline__ float4 d4(float4 t0, float4 t1, float4 t2, float4 t3)
 {
-    return make_float4(fmaf(PACT_C1, t2.x - t1.x, PACT_C2 * (t3.x - t0.x)), fmaf(PACT_C1, t2.y - t1.y, PACT_C2 * (t3.y - t0.y)),
-                       fmaf(PACT_C1, t2.z - t1.z, PACT_C2 * (t3.z - t0.z)), fmaf(PACT_C1, t2.w - t1.w, PACT_C2 * (t3.w - t0.w)));
+    return make_float4(d1(t0.x, t1.x, t2.x, t3.x), d1(t0.y, t1.y, t2.y, t3.y), d1(t0.z, t1.z, t2.z, t3.z), d1(t0.w, t1.w, t2.w, t3.w));
 }
 // along x on a quad c = f[0..3]: l = (f[-2], f[-1]), r = (f[4], f[5])
 __device__ __forceinline__ float4 dpx(float2 l, float4 c, float2 r)   // D+ : result at i + 1/2
 {
-    return make_float4(fmaf(PACT_C1, c.y - c.x, PACT_C2 * (c.z - l.y)), fmaf(PACT_C1, c.z - c.y, PACT_C2 * (c.w - c.x)),
-                       fmaf(PACT_C1, c.w - c.z, PACT_C2 * (r.x - c.y)), fmaf(PACT_C1, r.x - c.w, PACT_C2 * (r.y - c.z)));
+    return make_float4(d1(l.y, c.x, c.y, c.z), d1(c.x, c.y, c.z, c.w), d1(c.y, c.z, c.w, r.x), d1(c.z, c.w, r.x, r.y));
 }
 __device__ __forceinline__ float4 dmx(float2 l, float4 c, float2 r)   // D- : result at i
 {
-    return make_float4(fmaf(PACT_C1, c.x - l.y, PACT_C2 * (c.y - l.x)), fmaf(PACT_C1, c.y - c.x, PACT_C2 * (c.z - l.y)),
-                       fmaf(PACT_C1, c.z - c.y, PACT_C2 * (c.w - c.x)), fmaf(PACT_C1, c.w - c.z, PACT_C2 * (r.x - c.y)));
+    return make_float4(d1(l.x, l.y, c.x, c.y), d1(l.y, c.x, c.y, c.z), d1(c.x, c.y, c.z, c.w), d1(c.y, c.z, c.w, r.x));
 }
 
 __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
@@ -144,12 +170,10 @@ __device__ __forceinline__ void store_quad(float* p, float4 v, int x, int nx)
     if (x + 2 < nx) p[2] = v.z;
 }
 
-// ---- C-PML pieces (PML variant) -------------------------------------------------------------------
-struct PmlCtx {
-    bool bx, by;           // this CTA's box touches the x / y slabs
-};
-
-// slab column of grid column x (multiple of 4), or -1 ; x slab = [0,xl) U [xr,nxq)
+// ---- C-PML pieces ---------------------------------------------------------------------------------
+// Memory variables are stored slab-compressed, quad aligned in x (FusedArgs):
+//   axis x: [nz][ny][wx]   columns [0,xl) U [xr,nxq)      axis y: [nz][wyz][nxq]      axis z: [wyz][ny][nxq]
+// slab column of the quad starting at grid column x (multiple of 4), or -1
 __device__ __forceinline__ int xslab_col(const FusedArgs& a, int x)
 {
     if (x < 0 || x >= a.nxq) return -1;
@@ -157,6 +181,7 @@ __device__ __forceinline__ int xslab_col(const FusedArgs& a, int x)
     if (x >= a.xr) return a.xl + (x - a.xr);
     return -1;
 }
+// slab row of index i on an axis of length n (y or z), or -1
 __device__ __forceinline__ int yzslab_row(int i, int n, int P)
 {
     if (i < 0 || i >= n) return -1;
@@ -164,30 +189,121 @@ __device__ __forceinline__ int yzslab_row(int i, int n, int P)
     if (i >= n - 1 - P) return i - (n - 1 - P) + P;
     return -1;
 }
+__device__ __forceinline__ long long idx_x(const FusedArgs& a, int col, int y, int z) { return ((long long)z * a.ny + y) * a.wx + col; }
+__device__ __forceinline__ long long idx_y(const FusedArgs& a, int x, int row, int z) { return ((long long)z * a.wyz + row) * a.nxq + x; }
+__device__ __forceinline__ long long idx_z(const FusedArgs& a, int x, int y, int row) { return ((long long)row * a.ny + y) * a.nxq + x; }
+
+__device__ __forceinline__ float tab1(const float* t, int i, int n) { return (unsigned)i < (unsigned)n ? __ldg(t + i) : 0.0f; }
+// table values at x..x+3 ; 0 outside [0,n) (a = 0: no C-PML term ; b = 0 only ever multiplies zeros there)
 __device__ __forceinline__ float4 tab4(const float* t, int x, int n)
 {
-    // table values at x..x+3 ; outside [0,n): identity (a = 0 / b = 1 are chosen by the caller)
-    float4 v;
-    v.x = (unsigned)x < (unsigned)n ? __ldg(t + x) : 0.0f;
-    v.y = (unsigned)(x + 1) < (unsigned)n ? __ldg(t + x + 1) : 0.0f;
-    v.z = (unsigned)(x + 2) < (unsigned)n ? __ldg(t + x + 2) : 0.0f;
-    v.w = (unsigned)(x + 3) < (unsigned)n ? __ldg(t + x + 3) : 0.0f;
-    return v;
+    return make_float4(tab1(t, x, n), tab1(t, x + 1, n), tab1(t, x + 2, n), tab1(t, x + 3, n));
 }
 
+// Forward recursion on the thread's own quad (Eq. 46a / 46c with Eq. 38): m <- b m + a t ; returns t + m
+__device__ __forceinline__ float4 pml_fwd(const float* mi, float* mo, long long idx, float4 a4, float4 b4, float4 t, bool wr)
+{
+    const float4 m = fma4(b4, ldg4(mi + idx), a4 * t);
+    if (wr) stg4(mo + idx, m);
+    return t + m;
+}
+__device__ __forceinline__ float4 pml_fwd(const float* mi, float* mo, long long idx, float a1, float b1, float4 t, bool wr)
+{
+    const float4 m = fma4(b1, ldg4(mi + idx), a1 * t);
+    if (wr) stg4(mo + idx, m);
+    return t + m;
+}
+
+// Transposed recursion in tilde form (Eq. 61b / 61d-g): T <- b T + s at the
+// sample, and the differenced quantity is s + a T.  The a T part ("X") is needed at every tap of
+// the difference along the slab axis, so it is re-derived from the neighbours' old T.
+struct Taps8 { float2 l; float4 c; float2 r; };   // x-2,x-1 | x..x+3 | x+4,x+5
+
+// X along x for the row (y,z) of memory variable (Ti -> To); s = (l, c, r) are the samples at x-2..x+5
+__device__ __forceinline__ Taps8 adj_x(const FusedArgs& a, const float* __restrict__ Ti, float* __restrict__ To,
+                                       const float* __restrict__ ta, const float* __restrict__ tb,
+                                       int x, int y, int z, float2 l, float4 c, float2 r, bool wr)
+{
+    Taps8 X;
+    X.l = make_float2(0.0f, 0.0f); X.c = f4(0.0f); X.r = make_float2(0.0f, 0.0f);
+    const long long row = idx_x(a, 0, y, z);
+    int col = xslab_col(a, x);
+    if (col >= 0) {
+        const float4 Tn = fma4(tab4(tb, x, a.nx), ldg4(Ti + row + col), c);
+        if (wr) stg4(To + row + col, Tn);
+        X.c = tab4(ta, x, a.nx) * Tn;
+    }
+    col = xslab_col(a, x - 4);
+    if (col >= 0) {
+        const float4 T = ldg4(Ti + row + col);
+        X.l.x = tab1(ta, x - 2, a.nx) * fmaf(tab1(tb, x - 2, a.nx), T.z, l.x);
+        X.l.y = tab1(ta, x - 1, a.nx) * fmaf(tab1(tb, x - 1, a.nx), T.w, l.y);
+    }
+    col = xslab_col(a, x + 4);
+    if (col >= 0) {
+        const float4 T = ldg4(Ti + row + col);
+        X.r.x = tab1(ta, x + 4, a.nx) * fmaf(tab1(tb, x + 4, a.nx), T.x, r.x);
+        X.r.y = tab1(ta, x + 5, a.nx) * fmaf(tab1(tb, x + 5, a.nx), T.y, r.y);
+    }
+    return X;
+}
+// X along y: rows r0..r0+3 of plane z at the thread's quad ; tap `own` is the thread's own row.  Returns d4 of X.
+__device__ __forceinline__ float4 adj_y(const FusedArgs& a, const float* __restrict__ Ti, float* __restrict__ To,
+                                        const float* __restrict__ ta, const float* __restrict__ tb,
+                                        int x, int r0, int z, int own, float4 s0, float4 s1, float4 s2, float4 s3, bool wr)
+{
+    const float4 s[4] = {s0, s1, s2, s3};
+    float4 X[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        X[k] = f4(0.0f);
+        const int p = yzslab_row(r0 + k, a.ny, a.P);
+        if (p >= 0) {
+            const long long i = idx_y(a, x, p, z);
+            const float4 Tn = fma4(__ldg(tb + r0 + k), ldg4(Ti + i), s[k]);
+            if (wr && k == own) stg4(To + i, Tn);
+            X[k] = __ldg(ta + r0 + k) * Tn;
+        }
+    }
+    return d4(X[0], X[1], X[2], X[3]);
+}
+// X along z: planes z0..z0+3 at the thread's quad of row y
+__device__ __forceinline__ float4 adj_z(const FusedArgs& a, const float* __restrict__ Ti, float* __restrict__ To,
+                                        const float* __restrict__ ta, const float* __restrict__ tb,
+                                        int x, int y, int z0, int own, float4 s0, float4 s1, float4 s2, float4 s3, bool wr)
+{
+    const float4 s[4] = {s0, s1, s2, s3};
+    float4 X[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        X[k] = f4(0.0f);
+        const int p = yzslab_row(z0 + k, a.nz, a.P);
+        if (p >= 0) {
+            const long long i = idx_z(a, x, y, p);
+            const float4 Tn = fma4(__ldg(tb + z0 + k), ldg4(Ti + i), s[k]);
+            if (wr && k == own) stg4(To + i, Tn);
+            X[k] = __ldg(ta + z0 + k) * Tn;
+        }
+    }
+    return d4(X[0], X[1], X[2], X[3]);
+}
+// tilde-form update of an own-quad memory variable fed by the new value v: T <- b T + v
+__device__ __forceinline__ void adj_own(const float* Ti, float* To, long long i, float4 b4, float4 v) { stg4(To + i, fma4(b4, ldg4(Ti + i), v)); }
+__device__ __forceinline__ void adj_own(const float* Ti, float* To, long long i, float b1, float4 v) { stg4(To + i, fma4(b1, ldg4(Ti + i), v)); }
+
 // =================================================================================================
-// The fused step.  PML: the CTA applies the C-PML recursions (all CTAs of a launch share the
-// template; interior CTAs are launched with PML = false).  See DESIGN.md for the index algebra.
-template <bool PML>
+// The fused step.  MODE selects the C-PML code carried by the launch (FM_*); see DESIGN.md for the
+// index algebra.  Relative plane j <-> z = zb - 2 + j ; iteration `it` computes u(kk = zb - 2 + it)
+// and sigma(ks = kk - 2).
+template <int MODE>
 __global__ void __launch_bounds__(FT_NT, 1)
 k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUtensorMap tmS36,
         const __grid_constant__ CUtensorMap tmM40, const __grid_constant__ CUtensorMap tmM36, const FusedArgs a)
 {
     extern __shared__ __align__(1024) float sm[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(sm + FT_OFF_END);
-    uint64_t* barL = bars;        // [2]  s11, s22, s12 of plane j          -> slot j & 1
-    uint64_t* barE = bars + 2;    // [3]  s13, s23, rho, alpha of plane j ; s33 of plane j + 1 -> slot j % 3
-    uint64_t* barM = bars + 5;    // [3]  mu of plane j                     -> slot j % 3
+    uint64_t* barG = bars;        // [2]  everything first read by stage 1 of iteration c -> slot c & 1
+    uint64_t* barM = bars + 2;    // [3]  mu of plane j -> slot j % 3
 
     const int tid = threadIdx.x;
     int b = blockIdx.x;
@@ -212,6 +328,16 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
     const bool yin = (unsigned)y < (unsigned)a.ny;
     const bool m0 = yin && (unsigned)x < (unsigned)a.nx, m1 = yin && (unsigned)(x + 1) < (unsigned)a.nx;
     const bool m2 = yin && (unsigned)(x + 2) < (unsigned)a.nx, m3 = yin && (unsigned)(x + 3) < (unsigned)a.nx;
+    // the CTA's u region sticks out of the grid in x or y (then lanes are masked every plane)
+    const bool edge_xy = x0 == 0 || y0 == 0 || x0 + FT_TX + 4 > a.nx || y0 + FT_TY + 2 > a.ny;
+
+    // C-PML: does the CTA's region (plus the taps of the adjoint) touch the x / y slabs; own-quad slab positions
+    const bool pml = MODE != FM_PLAIN && a.P > 0;
+    const bool bx = pml && (x0 - 8 < a.xl || x0 + FT_TX + 8 > a.xr);
+    const bool by = pml && (y0 - 4 < a.P || y0 + FT_TY + 4 > a.ny - 1 - a.P);
+    const bool pok = pml && act1 && x >= 0 && x < a.nxq && yin;     // quad has memory-variable storage (given z in range)
+    const int colq = pok ? xslab_col(a, x) : -1;
+    const int prow = pok ? yzslab_row(y, a.ny, a.P) : -1;
 
     const float* in = a.in;
     const long long box = a.box;
@@ -227,22 +353,25 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
     const int cxm = x0 + PACT_HALO_X, cym = y0 + PACT_HALO_Y;
     const int cz0 = zb - 2 + PACT_HALO_Z;   // padded z of relative plane j = 0
 
-    auto issueL = [&](int j) {
-        uint64_t* bar = &barL[j & 1];
-        mbar_expect_tx(bar, 3 * FT_BOX * 4);
-        tma_plane(&tmS40, sm + FT_OFF_S11 + (j & 1) * FT_BOX, bar, cx40, cy40, cz0 + j, S11);
-        tma_plane(&tmS40, sm + FT_OFF_S22 + (j & 1) * FT_BOX, bar, cx40, cy40, cz0 + j, S22);
-        tma_plane(&tmS40, sm + FT_OFF_S12 + (j & 1) * FT_BOX, bar, cx40, cy40, cz0 + j, S12);
-    };
-    auto issueE = [&](int j) {
+    // E(j): s13, s23, rho, alpha of plane j -> slot j % 3
+    auto issueE = [&](int j, uint64_t* bar) {
         const int s = j % 3;
-        uint64_t* bar = &barE[s];
-        mbar_expect_tx(bar, (4 * FT_BOX + FT_UPL) * 4);
         tma_plane(&tmS40, sm + FT_OFF_S13 + s * FT_BOX, bar, cx40, cy40, cz0 + j, S13);
         tma_plane(&tmS40, sm + FT_OFF_S23 + s * FT_BOX, bar, cx40, cy40, cz0 + j, S23);
         tma_plane(&tmM40, sm + FT_OFF_RHO + s * FT_BOX, bar, cx40, cy40, cz0 + j, 2);
         tma_plane(&tmM40, sm + FT_OFF_ALP + s * FT_BOX, bar, cx40, cy40, cz0 + j, 3);
-        tma_plane(&tmS36, sm + FT_OFF_S33 + ((j + 1) & 1) * FT_UPL, bar, cx40, cy36, cz0 + j + 1, S33);
+    };
+    // group c = what stage 1 of iteration c reads for the first time:
+    //   s11, s22, s12 of plane c -> slot c & 1 ; E(c + 1) ; s33 of plane c + 2 -> slot c & 1 ; (c = 0: E(0) too)
+    auto issueG = [&](int c) {
+        uint64_t* bar = &barG[c & 1];
+        mbar_expect_tx(bar, (7 * FT_BOX + FT_UPL + (c == 0 ? 4 * FT_BOX : 0)) * 4);
+        tma_plane(&tmS40, sm + FT_OFF_S11 + (c & 1) * FT_BOX, bar, cx40, cy40, cz0 + c, S11);
+        tma_plane(&tmS40, sm + FT_OFF_S22 + (c & 1) * FT_BOX, bar, cx40, cy40, cz0 + c, S22);
+        tma_plane(&tmS40, sm + FT_OFF_S12 + (c & 1) * FT_BOX, bar, cx40, cy40, cz0 + c, S12);
+        issueE(c + 1, bar);
+        tma_plane(&tmS36, sm + FT_OFF_S33 + (c & 1) * FT_UPL, bar, cx40, cy36, cz0 + c + 2, S33);
+        if (c == 0) issueE(0, bar);
     };
     auto issueM = [&](int j) {
         uint64_t* bar = &barM[j % 3];
@@ -250,9 +379,9 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
         tma_plane(&tmM36, sm + FT_OFF_MU + (j % 3) * FT_MPL, bar, cxm, cym, cz0 + j, 1);
     };
 
-    if (tid == 0) { issueL(0); issueE(0); issueE(1); }
+    if (tid == 0) { issueG(0); issueG(1); }
 
-    // register windows along z (own column), relative plane j <-> z = zb - 2 + j
+    // register windows along z (own column)
     float4 w13a, w13b, w13c;          // s13 at kk-2, kk-1, kk
     float4 w23a, w23b, w23c;          // s23
     float4 w33a, w33b, w33c, w33d;    // s33 at kk-2, kk-1, kk, kk+1
@@ -276,25 +405,20 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
         uo3 = ld_ok ? ldg4(in + U3 * box + g) : z4;
         lam = so11 = so22 = so12 = z4;
     }
-    mbar_wait(&barE[0], 0);
 
-    const float sgn = a.sgn;
+    // coefficient scales: sign of the step and the 1/c2 of the unnormalised differences (d1)
+    const float kB = 2.0f * a.sgn * PACT_C2, kM = 4.0f * a.sgn * PACT_C2, kL = a.sgn * PACT_C2;
     const float* Rbase = sm + FT_OFF_RHO;
     const float* Abase = sm + FT_OFF_ALP;
+    const float* const* tb = reinterpret_cast<const float* const*>(a.tab);   // tab[3][4] flattened: tb[4 * axis + T_*]
 
     for (int it = 0; it < itn; ++it) {
         const int kk = zb - 2 + it;
-        if (tid == 0) {
-            if (it + 1 < itn) issueL(it + 1);
-            if (it + 2 <= itn) issueE(it + 2);
-            if (it <= itn - 2) issueM(it);
-        }
-        mbar_wait(&barL[it & 1], (it >> 1) & 1);
-        mbar_wait(&barE[(it + 1) % 3], ((it + 1) / 3) & 1);
-        if (it >= 1) mbar_wait(&barM[(it - 1) % 3], ((it - 1) / 3) & 1);
+        mbar_wait(&barG[it & 1], (it >> 1) & 1);
 
         const int s3 = it % 3, s3n = (it + 1) % 3;
         float4 f13 = z4, f23 = z4, f33 = z4;     // fresh window entries: s13, s23 at kk+1, s33 at kk+2
+        const bool zin = (unsigned)kk < (unsigned)a.nz;
         // ------------------------------------------------------------------ stage 1: u(kk)
         if (act1) {
             const float* P11 = sm + FT_OFF_S11 + (it & 1) * FT_BOX;
@@ -306,46 +430,111 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
             const float* PA = Abase + s3 * FT_BOX;
             f13 = ld4s(sm + FT_OFF_S13 + s3n * FT_BOX, q);
             f23 = ld4s(sm + FT_OFF_S23 + s3n * FT_BOX, q);
-            f33 = ld4s(sm + FT_OFF_S33 + (it & 1) * FT_UPL, uq);   // plane kk+2 = relative it+2 -> slot (it+2)&1
+            f33 = ld4s(sm + FT_OFF_S33 + (it & 1) * FT_UPL, uq);   // plane kk+2
+
+            const bool wr1 = inner && kk >= zb && kk < ze;          // this CTA owns u(x..x+3, y, kk)
+            // C-PML at this plane: z slab position of kk ; is any tap of the thread inside a slab
+            const int pz = (pml && zin) ? yzslab_row(kk, a.nz, a.P) : -1;
+            const bool bz = pml && (kk - 2 < a.P || kk + 2 >= a.nz - 1 - a.P);
+            const bool pml1 = (bx || by || bz) && pok && zin;
 
             // staggered coefficients (reading G10): J = 1 - dt alpha_b, B = dt/(h rho_b)
             const float4 r0 = ld4s(PR, q), a0 = ld4s(PA, q);
-            const float4 rxp = shl1(r0, PR[4 * q + 4]), axp = shl1(a0, PA[4 * q + 4]);
-            const float4 ryp = ld4s(PR, q + 10), ayp = ld4s(PA, q + 10);
-            const float4 rzp = ld4s(Rbase + s3n * FT_BOX, q), azp = ld4s(Abase + s3n * FT_BOX, q);
             const float4 one = f4(1.0f), mh = f4(-0.5f);
-            const float4 J1 = fma4(mh, a0 + axp, one), J2 = fma4(mh, a0 + ayp, one), J3 = fma4(mh, a0 + azp, one);
-            const float4 B1 = (2.0f * sgn) * rcp4(r0 + rxp), B2 = (2.0f * sgn) * rcp4(r0 + ryp), B3 = (2.0f * sgn) * rcp4(r0 + rzp);
-
-            // nine derivatives of sigma (Eq. 46b)
-            const float4 c11 = ld4s(P11, q), c12 = ld4s(P12, q), c22 = ld4s(P22, q);
-            float4 d1 = dpx(ld2s(P11, 4 * q - 2), c11, ld2s(P11, 4 * q + 4));                       // D+x s11
-            d1 = d1 + d4(ld4s(P12, q - 20), ld4s(P12, q - 10), c12, ld4s(P12, q + 10));             // D-y s12
-            d1 = d1 + d4(w13a, w13b, w13c, f13);                                                    // D-z s13
-            float4 d2 = dmx(ld2s(P12, 4 * q - 2), c12, ld2s(P12, 4 * q + 4));                       // D-x s12
-            d2 = d2 + d4(ld4s(P22, q - 10), c22, ld4s(P22, q + 10), ld4s(P22, q + 20));             // D+y s22
-            d2 = d2 + d4(w23a, w23b, w23c, f23);                                                    // D-z s23
-            float4 d3 = dmx(ld2s(P13, 4 * q - 2), w13c, ld2s(P13, 4 * q + 4));                      // D-x s13
-            d3 = d3 + d4(ld4s(P23, q - 20), ld4s(P23, q - 10), w23c, ld4s(P23, q + 10));            // D-y s23
-            d3 = d3 + d4(w33b, w33c, w33d, f33);                                                    // D+z s33
-
-            float4 n1 = fma4(J1, uo1, B1 * d1), n2 = fma4(J2, uo2, B2 * d2), n3 = fma4(J3, uo3, B3 * d3);
-            const bool zin = (unsigned)kk < (unsigned)a.nz;
-            if (!(zin && m0)) { n1.x = 0.0f; n2.x = 0.0f; n3.x = 0.0f; }
-            if (!(zin && m1)) { n1.y = 0.0f; n2.y = 0.0f; n3.y = 0.0f; }
-            if (!(zin && m2)) { n1.z = 0.0f; n2.z = 0.0f; n3.z = 0.0f; }
-            if (!(zin && m3)) { n1.w = 0.0f; n2.w = 0.0f; n3.w = 0.0f; }
+            const float4 c12 = ld4s(P12, q);
+            float4 n1, n2, n3;
+            {   // ---- u1 at (x+1/2, y, z): D+x s11, D-y s12, D-z s13
+                const float4 c11 = ld4s(P11, q);
+                const float2 l = ld2s(P11, 4 * q - 2), rr = ld2s(P11, 4 * q + 4);
+                const float4 ya = ld4s(P12, q - 20), yb = ld4s(P12, q - 10), yd = ld4s(P12, q + 10);
+                float4 t1 = dpx(l, c11, rr), t2 = d4(ya, yb, c12, yd), t3 = d4(w13a, w13b, w13c, f13);
+                if (MODE == FM_FWD && pml1) {
+                    if (colq >= 0) t1 = pml_fwd(a.mvi[0], a.mvo[0], idx_x(a, colq, y, kk), tab4(tb[T_A_HALF], x, a.nx), tab4(tb[T_B_HALF], x, a.nx), t1, wr1);
+                    if (prow >= 0) t2 = pml_fwd(a.mvi[1], a.mvo[1], idx_y(a, x, prow, kk), __ldg(tb[4 + T_A_INT] + y), __ldg(tb[4 + T_B_INT] + y), t2, wr1);
+                    if (pz >= 0) t3 = pml_fwd(a.mvi[2], a.mvo[2], idx_z(a, x, y, pz), __ldg(tb[8 + T_A_INT] + kk), __ldg(tb[8 + T_B_INT] + kk), t3, wr1);
+                }
+                if (MODE == FM_ADJ && pml1) {
+                    if (bx) { const Taps8 X = adj_x(a, a.mvi[9], a.mvo[9], tb[T_A_INT], tb[T_B_INT], x, y, kk, l, c11, rr, wr1); t1 = t1 + dpx(X.l, X.c, X.r); }
+                    if (by) t2 = t2 + adj_y(a, a.mvi[10], a.mvo[10], tb[4 + T_A_HALF], tb[4 + T_B_HALF], x, y - 2, kk, 2, ya, yb, c12, yd, wr1);
+                    if (bz) t3 = t3 + adj_z(a, a.mvi[11], a.mvo[11], tb[8 + T_A_HALF], tb[8 + T_B_HALF], x, y, kk - 2, 2, w13a, w13b, w13c, f13, wr1);
+                }
+                const float4 rxp = shl1(r0, PR[4 * q + 4]), axp = shl1(a0, PA[4 * q + 4]);
+                n1 = fma4(fma4(mh, a0 + axp, one), uo1, (kB * rcp4(r0 + rxp)) * (t1 + t2 + t3));
+            }
+            {   // ---- u2 at (x, y+1/2, z): D-x s12, D+y s22, D-z s23
+                const float2 l = ld2s(P12, 4 * q - 2), rr = ld2s(P12, 4 * q + 4);
+                const float4 yb = ld4s(P22, q - 10), c22 = ld4s(P22, q), yc = ld4s(P22, q + 10), yd = ld4s(P22, q + 20);
+                float4 t1 = dmx(l, c12, rr), t2 = d4(yb, c22, yc, yd), t3 = d4(w23a, w23b, w23c, f23);
+                if (MODE == FM_FWD && pml1) {
+                    if (colq >= 0) t1 = pml_fwd(a.mvi[3], a.mvo[3], idx_x(a, colq, y, kk), tab4(tb[T_A_INT], x, a.nx), tab4(tb[T_B_INT], x, a.nx), t1, wr1);
+                    if (prow >= 0) t2 = pml_fwd(a.mvi[4], a.mvo[4], idx_y(a, x, prow, kk), __ldg(tb[4 + T_A_HALF] + y), __ldg(tb[4 + T_B_HALF] + y), t2, wr1);
+                    if (pz >= 0) t3 = pml_fwd(a.mvi[5], a.mvo[5], idx_z(a, x, y, pz), __ldg(tb[8 + T_A_INT] + kk), __ldg(tb[8 + T_B_INT] + kk), t3, wr1);
+                }
+                if (MODE == FM_ADJ && pml1) {
+                    if (bx) { const Taps8 X = adj_x(a, a.mvi[12], a.mvo[12], tb[T_A_HALF], tb[T_B_HALF], x, y, kk, l, c12, rr, wr1); t1 = t1 + dmx(X.l, X.c, X.r); }
+                    if (by) t2 = t2 + adj_y(a, a.mvi[13], a.mvo[13], tb[4 + T_A_INT], tb[4 + T_B_INT], x, y - 1, kk, 1, yb, c22, yc, yd, wr1);
+                    if (bz) t3 = t3 + adj_z(a, a.mvi[14], a.mvo[14], tb[8 + T_A_HALF], tb[8 + T_B_HALF], x, y, kk - 2, 2, w23a, w23b, w23c, f23, wr1);
+                }
+                const float4 ryp = ld4s(PR, q + 10), ayp = ld4s(PA, q + 10);
+                n2 = fma4(fma4(mh, a0 + ayp, one), uo2, (kB * rcp4(r0 + ryp)) * (t1 + t2 + t3));
+            }
+            {   // ---- u3 at (x, y, z+1/2): D-x s13, D-y s23, D+z s33
+                const float2 l = ld2s(P13, 4 * q - 2), rr = ld2s(P13, 4 * q + 4);
+                const float4 ya = ld4s(P23, q - 20), yb = ld4s(P23, q - 10), yd = ld4s(P23, q + 10);
+                float4 t1 = dmx(l, w13c, rr), t2 = d4(ya, yb, w23c, yd), t3 = d4(w33b, w33c, w33d, f33);
+                if (MODE == FM_FWD && pml1) {
+                    if (colq >= 0) t1 = pml_fwd(a.mvi[6], a.mvo[6], idx_x(a, colq, y, kk), tab4(tb[T_A_INT], x, a.nx), tab4(tb[T_B_INT], x, a.nx), t1, wr1);
+                    if (prow >= 0) t2 = pml_fwd(a.mvi[7], a.mvo[7], idx_y(a, x, prow, kk), __ldg(tb[4 + T_A_INT] + y), __ldg(tb[4 + T_B_INT] + y), t2, wr1);
+                    if (pz >= 0) t3 = pml_fwd(a.mvi[8], a.mvo[8], idx_z(a, x, y, pz), __ldg(tb[8 + T_A_HALF] + kk), __ldg(tb[8 + T_B_HALF] + kk), t3, wr1);
+                }
+                if (MODE == FM_ADJ && pml1) {
+                    if (bx) { const Taps8 X = adj_x(a, a.mvi[15], a.mvo[15], tb[T_A_HALF], tb[T_B_HALF], x, y, kk, l, w13c, rr, wr1); t1 = t1 + dmx(X.l, X.c, X.r); }
+                    if (by) t2 = t2 + adj_y(a, a.mvi[16], a.mvo[16], tb[4 + T_A_HALF], tb[4 + T_B_HALF], x, y - 2, kk, 2, ya, yb, w23c, yd, wr1);
+                    if (bz) t3 = t3 + adj_z(a, a.mvi[17], a.mvo[17], tb[8 + T_A_INT], tb[8 + T_B_INT], x, y, kk - 1, 1, w33b, w33c, w33d, f33, wr1);
+                }
+                const float4 rzp = ld4s(Rbase + s3n * FT_BOX, q), azp = ld4s(Abase + s3n * FT_BOX, q);
+                n3 = fma4(fma4(mh, a0 + azp, one), uo3, (kB * rcp4(r0 + rzp)) * (t1 + t2 + t3));
+            }
+            if (edge_xy || !zin) {
+                if (!(zin && m0)) { n1.x = 0.0f; n2.x = 0.0f; n3.x = 0.0f; }
+                if (!(zin && m1)) { n1.y = 0.0f; n2.y = 0.0f; n3.y = 0.0f; }
+                if (!(zin && m2)) { n1.z = 0.0f; n2.z = 0.0f; n3.z = 0.0f; }
+                if (!(zin && m3)) { n1.w = 0.0f; n2.w = 0.0f; n3.w = 0.0f; }
+            }
             const int sl = it % FT_RING;
             *reinterpret_cast<float4*>(sm + FT_OFF_UR + (0 * FT_RING + sl) * FT_UPL + 4 * uq) = n1;
             *reinterpret_cast<float4*>(sm + FT_OFF_UR + (1 * FT_RING + sl) * FT_UPL + 4 * uq) = n2;
             *reinterpret_cast<float4*>(sm + FT_OFF_UR + (2 * FT_RING + sl) * FT_UPL + 4 * uq) = n3;
             const long long g = (long long)kk * a.sz + gxy;
-            if (inner && kk >= zb && kk < ze) {
+            if (wr1) {
                 store_quad(a.out + U1 * box + g, n1, x, a.nx);
                 store_quad(a.out + U2 * box + g, n2, x, a.nx);
                 store_quad(a.out + U3 * box + g, n3, x, a.nx);
+                if (MODE == FM_ADJ && pml1) {   // phi_bar (tilde form) fed by the new u_bar: Eq. 61c,e in scaled variables
+                    if (colq >= 0) {
+                        const long long i = idx_x(a, colq, y, kk);
+                        const float4 bi = tab4(tb[T_B_INT], x, a.nx);
+                        adj_own(a.mvi[0], a.mvo[0], i, tab4(tb[T_B_HALF], x, a.nx), n1);
+                        adj_own(a.mvi[3], a.mvo[3], i, bi, n2);
+                        adj_own(a.mvi[6], a.mvo[6], i, bi, n3);
+                    }
+                    if (prow >= 0) {
+                        const long long i = idx_y(a, x, prow, kk);
+                        const float bi = __ldg(tb[4 + T_B_INT] + y);
+                        adj_own(a.mvi[1], a.mvo[1], i, bi, n1);
+                        adj_own(a.mvi[4], a.mvo[4], i, __ldg(tb[4 + T_B_HALF] + y), n2);
+                        adj_own(a.mvi[7], a.mvo[7], i, bi, n3);
+                    }
+                    if (pz >= 0) {
+                        const long long i = idx_z(a, x, y, pz);
+                        const float bi = __ldg(tb[8 + T_B_INT] + kk);
+                        adj_own(a.mvi[2], a.mvo[2], i, bi, n1);
+                        adj_own(a.mvi[5], a.mvo[5], i, bi, n2);
+                        adj_own(a.mvi[8], a.mvo[8], i, __ldg(tb[8 + T_B_HALF] + kk), n3);
+                    }
+                }
             }
-            // u_old of the next plane (in flight during stage 2 and the next waits)
+            // u_old of the next plane (in flight during stage 2)
             if (ld_ok && it + 1 < itn) {
                 uo1 = ldg4(in + U1 * box + g + a.sz);
                 uo2 = ldg4(in + U2 * box + g + a.sz);
@@ -353,6 +542,12 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
             }
         }
         __syncthreads();
+        // every thread is past stage 1 of `it` and stage 2 of `it - 1`: refill the slots they freed
+        if (tid == 0) {
+            if (it + 2 < itn) issueG(it + 2);
+            if (it + 2 <= itn) issueM(it);   // mu(j) is read by stage 2 of iterations j + 1 and j + 2
+        }
+        if (it >= 1) mbar_wait(&barM[(it - 1) % 3], ((it - 1) / 3) & 1);
         // ------------------------------------------------------------------ stage 2: sigma(ks), ks = kk - 2
         const int ks = kk - 2;
         if (inner && it >= 4) {
@@ -362,27 +557,72 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
             const float* U3p = sm + FT_OFF_UR + 2 * FT_RING * FT_UPL;
             const int p0 = (j % FT_RING) * FT_UPL, pm1 = ((j + 4) % FT_RING) * FT_UPL, pm2 = ((j + 3) % FT_RING) * FT_UPL;
             const int pp1 = ((j + 1) % FT_RING) * FT_UPL, pp2 = ((j + 2) % FT_RING) * FT_UPL;
-            const float4 c1 = ld4s(U1p + p0, uq), c2 = ld4s(U2p + p0, uq), c3 = ld4s(U3p + p0, uq);
-            float4 e11 = dmx(ld2s(U1p + p0, 4 * uq - 2), c1, ld2s(U1p + p0, 4 * uq + 4));                        // D-x u1
-            float4 g12 = d4(ld4s(U1p + p0, uq - 10), c1, ld4s(U1p + p0, uq + 10), ld4s(U1p + p0, uq + 20));     // D+y u1
-            float4 g13 = d4(ld4s(U1p + pm1, uq), c1, ld4s(U1p + pp1, uq), ld4s(U1p + pp2, uq));                 // D+z u1
-            float4 g21 = dpx(ld2s(U2p + p0, 4 * uq - 2), c2, ld2s(U2p + p0, 4 * uq + 4));                        // D+x u2
-            float4 e22 = d4(ld4s(U2p + p0, uq - 20), ld4s(U2p + p0, uq - 10), c2, ld4s(U2p + p0, uq + 10));     // D-y u2
-            float4 g23 = d4(ld4s(U2p + pm1, uq), c2, ld4s(U2p + pp1, uq), ld4s(U2p + pp2, uq));                 // D+z u2
-            float4 g31 = dpx(ld2s(U3p + p0, 4 * uq - 2), c3, ld2s(U3p + p0, 4 * uq + 4));                        // D+x u3
-            float4 g32 = d4(ld4s(U3p + p0, uq - 10), c3, ld4s(U3p + p0, uq + 10), ld4s(U3p + p0, uq + 20));     // D+y u3
-            float4 e33 = d4(ld4s(U3p + pm2, uq), ld4s(U3p + pm1, uq), c3, ld4s(U3p + pp1, uq));                 // D-z u3
+            const int pz = pml ? yzslab_row(ks, a.nz, a.P) : -1;
+            const bool bz = pml && (ks - 2 < a.P || ks + 2 >= a.nz - 1 - a.P);
+            const bool pml2 = bx || by || bz;       // inner threads have storage: 0 <= x < nx, 0 <= y < ny, zb <= ks < ze
+            float4 e11, e22, e33, g12, g21, g13, g31, g23, g32;
+            {   // ---- derivatives of u1: D-x (e11), D+y (g12), D+z (g13)
+                const float4 c = ld4s(U1p + p0, uq);
+                const float2 l = ld2s(U1p + p0, 4 * uq - 2), rr = ld2s(U1p + p0, 4 * uq + 4);
+                const float4 ya = ld4s(U1p + p0, uq - 10), yc = ld4s(U1p + p0, uq + 10), yd = ld4s(U1p + p0, uq + 20);
+                const float4 za = ld4s(U1p + pm1, uq), zc = ld4s(U1p + pp1, uq), zd = ld4s(U1p + pp2, uq);
+                e11 = dmx(l, c, rr); g12 = d4(ya, c, yc, yd); g13 = d4(za, c, zc, zd);
+                if (MODE == FM_FWD && pml2) {
+                    if (colq >= 0) e11 = pml_fwd(a.mvi[9], a.mvo[9], idx_x(a, colq, y, ks), tab4(tb[T_A_INT], x, a.nx), tab4(tb[T_B_INT], x, a.nx), e11, true);
+                    if (prow >= 0) g12 = pml_fwd(a.mvi[10], a.mvo[10], idx_y(a, x, prow, ks), __ldg(tb[4 + T_A_HALF] + y), __ldg(tb[4 + T_B_HALF] + y), g12, true);
+                    if (pz >= 0) g13 = pml_fwd(a.mvi[11], a.mvo[11], idx_z(a, x, y, pz), __ldg(tb[8 + T_A_HALF] + ks), __ldg(tb[8 + T_B_HALF] + ks), g13, true);
+                }
+                if (MODE == FM_ADJ && pml2) {
+                    if (bx) { const Taps8 X = adj_x(a, a.mvi[0], nullptr, tb[T_A_HALF], tb[T_B_HALF], x, y, ks, l, c, rr, false); e11 = e11 + dmx(X.l, X.c, X.r); }
+                    if (by) g12 = g12 + adj_y(a, a.mvi[1], nullptr, tb[4 + T_A_INT], tb[4 + T_B_INT], x, y - 1, ks, 1, ya, c, yc, yd, false);
+                    if (bz) g13 = g13 + adj_z(a, a.mvi[2], nullptr, tb[8 + T_A_INT], tb[8 + T_B_INT], x, y, ks - 1, 1, za, c, zc, zd, false);
+                }
+            }
+            {   // ---- derivatives of u2: D+x (g21), D-y (e22), D+z (g23)
+                const float4 c = ld4s(U2p + p0, uq);
+                const float2 l = ld2s(U2p + p0, 4 * uq - 2), rr = ld2s(U2p + p0, 4 * uq + 4);
+                const float4 ya = ld4s(U2p + p0, uq - 20), yb = ld4s(U2p + p0, uq - 10), yd = ld4s(U2p + p0, uq + 10);
+                const float4 za = ld4s(U2p + pm1, uq), zc = ld4s(U2p + pp1, uq), zd = ld4s(U2p + pp2, uq);
+                g21 = dpx(l, c, rr); e22 = d4(ya, yb, c, yd); g23 = d4(za, c, zc, zd);
+                if (MODE == FM_FWD && pml2) {
+                    if (colq >= 0) g21 = pml_fwd(a.mvi[12], a.mvo[12], idx_x(a, colq, y, ks), tab4(tb[T_A_HALF], x, a.nx), tab4(tb[T_B_HALF], x, a.nx), g21, true);
+                    if (prow >= 0) e22 = pml_fwd(a.mvi[13], a.mvo[13], idx_y(a, x, prow, ks), __ldg(tb[4 + T_A_INT] + y), __ldg(tb[4 + T_B_INT] + y), e22, true);
+                    if (pz >= 0) g23 = pml_fwd(a.mvi[14], a.mvo[14], idx_z(a, x, y, pz), __ldg(tb[8 + T_A_HALF] + ks), __ldg(tb[8 + T_B_HALF] + ks), g23, true);
+                }
+                if (MODE == FM_ADJ && pml2) {
+                    if (bx) { const Taps8 X = adj_x(a, a.mvi[3], nullptr, tb[T_A_INT], tb[T_B_INT], x, y, ks, l, c, rr, false); g21 = g21 + dpx(X.l, X.c, X.r); }
+                    if (by) e22 = e22 + adj_y(a, a.mvi[4], nullptr, tb[4 + T_A_HALF], tb[4 + T_B_HALF], x, y - 2, ks, 2, ya, yb, c, yd, false);
+                    if (bz) g23 = g23 + adj_z(a, a.mvi[5], nullptr, tb[8 + T_A_INT], tb[8 + T_B_INT], x, y, ks - 1, 1, za, c, zc, zd, false);
+                }
+            }
+            {   // ---- derivatives of u3: D+x (g31), D+y (g32), D-z (e33)
+                const float4 c = ld4s(U3p + p0, uq);
+                const float2 l = ld2s(U3p + p0, 4 * uq - 2), rr = ld2s(U3p + p0, 4 * uq + 4);
+                const float4 ya = ld4s(U3p + p0, uq - 10), yc = ld4s(U3p + p0, uq + 10), yd = ld4s(U3p + p0, uq + 20);
+                const float4 za = ld4s(U3p + pm2, uq), zb_ = ld4s(U3p + pm1, uq), zd = ld4s(U3p + pp1, uq);
+                g31 = dpx(l, c, rr); g32 = d4(ya, c, yc, yd); e33 = d4(za, zb_, c, zd);
+                if (MODE == FM_FWD && pml2) {
+                    if (colq >= 0) g31 = pml_fwd(a.mvi[15], a.mvo[15], idx_x(a, colq, y, ks), tab4(tb[T_A_HALF], x, a.nx), tab4(tb[T_B_HALF], x, a.nx), g31, true);
+                    if (prow >= 0) g32 = pml_fwd(a.mvi[16], a.mvo[16], idx_y(a, x, prow, ks), __ldg(tb[4 + T_A_HALF] + y), __ldg(tb[4 + T_B_HALF] + y), g32, true);
+                    if (pz >= 0) e33 = pml_fwd(a.mvi[17], a.mvo[17], idx_z(a, x, y, pz), __ldg(tb[8 + T_A_INT] + ks), __ldg(tb[8 + T_B_INT] + ks), e33, true);
+                }
+                if (MODE == FM_ADJ && pml2) {
+                    if (bx) { const Taps8 X = adj_x(a, a.mvi[6], nullptr, tb[T_A_INT], tb[T_B_INT], x, y, ks, l, c, rr, false); g31 = g31 + dpx(X.l, X.c, X.r); }
+                    if (by) g32 = g32 + adj_y(a, a.mvi[7], nullptr, tb[4 + T_A_INT], tb[4 + T_B_INT], x, y - 1, ks, 1, ya, c, yc, yd, false);
+                    if (bz) e33 = e33 + adj_z(a, a.mvi[8], nullptr, tb[8 + T_A_HALF], tb[8 + T_B_HALF], x, y, ks - 2, 2, za, zb_, c, zd, false);
+                }
+            }
 
             // Lame coefficients: lambda, 2 mu at the node; 4-point harmonic mu at shear points (reading G10)
             const float* M0 = sm + FT_OFF_MU + (j % 3) * FT_MPL;
             const float* M1 = sm + FT_OFF_MU + ((j + 1) % 3) * FT_MPL;
             const float4 i0 = ld4s(M0, mq), iy = ld4s(M0, mq + 9), iz = ld4s(M1, mq), iyz = ld4s(M1, mq + 9);
             const float4 ix = shl1(i0, M0[4 * mq + 4]), ixy = shl1(iy, M0[4 * mq + 40]), ixz = shl1(iz, M1[4 * mq + 4]);
-            const float4 mn2 = (2.0f * sgn) * rcp4(i0);
-            const float4 mxy = (4.0f * sgn) * rcp4((i0 + ix) + (iy + ixy));
-            const float4 mxz = (4.0f * sgn) * rcp4((i0 + ix) + (iz + ixz));
-            const float4 myz = (4.0f * sgn) * rcp4((i0 + iy) + (iz + iyz));
-            const float4 ldiv = (sgn * lam) * (e11 + e22 + e33);
+            const float4 mn2 = kB * rcp4(i0);
+            const float4 mxy = kM * rcp4((i0 + ix) + (iy + ixy));
+            const float4 mxz = kM * rcp4((i0 + ix) + (iz + ixz));
+            const float4 myz = kM * rcp4((i0 + iy) + (iz + iyz));
+            const float4 ldiv = (kL * lam) * (e11 + e22 + e33);
             const float4 n11 = so11 + fma4(mn2, e11, ldiv);
             const float4 n22 = so22 + fma4(mn2, e22, ldiv);
             const float4 n33 = w33a + fma4(mn2, e33, ldiv);
@@ -408,6 +648,5 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
         w13a = w13b; w13b = w13c; w13c = f13;
         w23a = w23b; w23b = w23c; w23c = f23;
         w33a = w33b; w33b = w33c; w33c = w33d; w33d = f33;
-        __syncthreads();
     }
 }

@@ -481,8 +481,9 @@ static int ensure_fused(pact_ctx* c)
     if ((rc = make_map(c, enc, &c->tmS36[1], baseB, NFIELD, FT_BW, FT_UH))) return rc;
     if ((rc = make_map(c, enc, &c->tmM40, baseM, 4, FT_BW, FT_BH))) return rc;
     if ((rc = make_map(c, enc, &c->tmM36, baseM, 4, FT_MW, FT_MH))) return rc;
-    CK(cudaFuncSetAttribute(k_fused<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
-    CK(cudaFuncSetAttribute(k_fused<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
+    CK(cudaFuncSetAttribute(k_fused<FM_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
+    CK(cudaFuncSetAttribute(k_fused<FM_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
+    CK(cudaFuncSetAttribute(k_fused<FM_ADJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
     fa.mat = g.Ll;
     c->fused_ready = true;
     return PACT_OK;
@@ -499,19 +500,27 @@ static void fused_step(pact_ctx* c, Launcher& ln, int cur, float sgn, int kind)
     for (int k = 0; k < 18; ++k) { fa.mvi[k] = c->mvbuf[cur][k]; fa.mvo[k] = c->mvbuf[1 - cur][k]; }
     int zc = c->zchunk;
     if (zc <= 0) {
-        // enough CTAs for ~7 waves of 148 SMs, chunks no shorter than 32 planes
+        // z chunks: one CTA per SM and 4 start-up planes per chunk; take the chunk count that minimises
+        // waves x (planes per chunk + 4), chunks no shorter than 32 planes
         const int tiles = fa.ntx * fa.nty;
-        int nzc = std::max(1, (7 * 148 + tiles - 1) / tiles);
-        zc = std::max(32, (fa.nz + nzc - 1) / nzc);
+        long long best = -1;
+        for (int nzc = 1; nzc <= std::max(1, fa.nz / 32); ++nzc) {
+            const int z = (fa.nz + nzc - 1) / nzc;
+            const long long ctas = (long long)tiles * ((fa.nz + z - 1) / z);
+            const long long cost = ((ctas + 147) / 148) * (z + 4);
+            if (best < 0 || cost < best) { best = cost; zc = z; }
+        }
     }
-    zc = std::min(zc, fa.nz);
+    zc = std::max(1, std::min(zc, fa.nz));
     fa.zc = zc; fa.nzc = (fa.nz + zc - 1) / zc;
     const int grid = fa.ntx * fa.nty * fa.nzc;
     cudaStream_t st = c->stream;
-    if (fa.P > 0)
-        ln.run(kind, [&] { k_fused<true><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM40, c->tmM36, fa); });
+    if (fa.P == 0)
+        ln.run(kind, [&] { k_fused<FM_PLAIN><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM40, c->tmM36, fa); });
+    else if (sgn > 0.0f)
+        ln.run(kind, [&] { k_fused<FM_FWD><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM40, c->tmM36, fa); });
     else
-        ln.run(kind, [&] { k_fused<false><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM40, c->tmM36, fa); });
+        ln.run(kind, [&] { k_fused<FM_ADJ><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM40, c->tmM36, fa); });
 }
 
 // Eq. 58 right to left: tau, then for m = 0..M-1 { Theta ; W' unless m = M-1 }

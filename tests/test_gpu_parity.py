@@ -27,16 +27,17 @@ def torch_cuda():
     return torch
 
 
-def gpu_ops(torch, prob, variant=0, graph=-1):
+def gpu_ops(torch, prob, variant=0, graph=-1, zchunk=0):
     from paper_1709_02733_b200.binding import Pact
     ctx = Pact.from_problem(prob)
     ctx.set_option("variant", variant)
     ctx.set_option("graph", graph)
+    ctx.set_option("zchunk", zchunk)
     return ctx
 
 
-def run_pair(torch, prob, x, y, variant=0, graph=-1):
-    ctx = gpu_ops(torch, prob, variant, graph)
+def run_pair(torch, prob, x, y, variant=0, graph=-1, zchunk=0):
+    ctx = gpu_ops(torch, prob, variant, graph, zchunk)
     xd = torch.from_numpy(np.ascontiguousarray(x, dtype=np.float32)).cuda()
     yd = torch.from_numpy(np.ascontiguousarray(y, dtype=np.float32)).cuda()
     Hx = ctx.forward(xd).cpu().numpy()
@@ -55,13 +56,14 @@ def oracle_pair(prob, x, y):
     return Hx, Hty
 
 
-VARIANTS = [1]
+VARIANTS = [1, 2]    # 1: plain two-kernel path ; 2: fused single-pass path (the default)
 
-# sizes span several 32x8x2 / 64x16 tiles plus ragged tails in every axis
+# sizes span several 32x8x2 (plain) / 32x32 (fused) tiles plus ragged tails in every axis
 RANDOM_CASES = [
     dict(nx=45, ny=37, nz=41, nt=40, npml=5, L=19, seed=1, lossy=True),
     dict(nx=70, ny=34, nz=29, nt=30, npml=4, L=11, seed=2, lossy=True),
     dict(nx=33, ny=66, nz=20, nt=25, npml=0, L=9, seed=3, lossy=False),
+    dict(nx=75, ny=70, nz=23, nt=22, npml=6, L=13, seed=21, lossy=True),     # 3 x 3 fused tiles, ragged
     dict(nx=8, ny=8, nz=8, nt=12, npml=0, L=3, seed=4, lossy=True),          # minimum grid
     dict(nx=16, ny=17, nz=18, nt=20, npml=4, L=5, seed=5, lossy=True),       # 2*npml+8 == nx: thickest legal PML
 ]
@@ -106,6 +108,18 @@ def test_config2_truncated(torch_cuda, variant):
     y = rng.standard_normal((prob.prm.nt, prob.L))
     Hx, Hty = run_pair(torch_cuda, prob, prob.p0, y, variant)
     Hx_o, Hty_o = oracle_pair(prob, prob.p0, y)
+    assert rel_l2(Hx, Hx_o) <= TOL_L2
+    assert rel_l2(Hty, Hty_o) <= TOL_L2
+
+
+@pytest.mark.parametrize("zchunk", [1, 5, 16])
+def test_fused_z_chunking(torch_cuda, zchunk):
+    """The fused kernel marches z in chunks that recompute 2 planes of u on either side: any chunk
+    length gives the same operator (several chunks intersect the z slabs of the C-PML here)."""
+    prob = synth.random_problem(nx=40, ny=36, nz=45, nt=24, npml=5, L=9, seed=22, lossy=True)
+    x, y = synth.random_vectors(prob, seed=22)
+    Hx, Hty = run_pair(torch_cuda, prob, x, y, variant=2, zchunk=zchunk)
+    Hx_o, Hty_o = oracle_pair(prob, x, y)
     assert rel_l2(Hx, Hx_o) <= TOL_L2
     assert rel_l2(Hty, Hty_o) <= TOL_L2
 
