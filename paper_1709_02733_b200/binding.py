@@ -13,7 +13,8 @@ from pathlib import Path
 import numpy as np
 
 _HERE = Path(__file__).resolve().parent
-_LIBPATH = _HERE / "libpact.so"
+import os as _os
+_LIBPATH = Path(_os.environ.get("PACT_LIBRARY", _HERE / "libpact.so"))   # override: another build of the same library
 
 PACT_OK = 0
 ERRORS = {-1: "PACT_EINVAL", -2: "PACT_ECFL", -3: "PACT_ERCV", -4: "PACT_EMATERIAL", -5: "PACT_ENOMEM",

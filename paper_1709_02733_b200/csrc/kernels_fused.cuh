@@ -40,7 +40,9 @@
 #define FT_MW 36                      // mu box: tile + 1 (rounded up to a quad) in x
 #define FT_MH 33                      //         tile + 1 in y
 #define FT_MPL 1216                   // floats per mu plane buffer (36*33 = 1188, padded to 128 B)
+#ifndef FT_RING
 #define FT_RING 5                     // u planes kept for stage 2: ks-2 .. ks+2
+#endif
 
 // shared memory map (floats)
 #define FT_OFF_S11 0
@@ -54,7 +56,12 @@
 #define FT_OFF_MU (FT_OFF_S33 + 2 * FT_UPL)
 #define FT_OFF_UR (FT_OFF_MU + 3 * FT_MPL)
 #define FT_OFF_END (FT_OFF_UR + 3 * FT_RING * FT_UPL)
-#define FT_SMEM_BYTES (FT_OFF_END * 4 + 64)   // + 8 mbarriers
+#define FT_TABW 48                     // x / y C-PML table window: tile - 8 .. tile + 39
+#define FT_ZRING 16                   // z C-PML table ring (planes)
+#define FT_OFF_XT (FT_OFF_END + 16)   // after 8 mbarriers (64 B)
+#define FT_OFF_YT (FT_OFF_XT + 4 * FT_TABW)
+#define FT_OFF_ZT (FT_OFF_YT + 4 * FT_TABW)
+#define FT_SMEM_BYTES ((FT_OFF_ZT + 4 * FT_ZRING) * 4)
 
 // kernel modes: which C-PML code a launch carries (CTAs away from the slabs skip it at run time)
 #define FM_PLAIN 0     // no C-PML (npml = 0)
@@ -113,6 +120,13 @@ __device__ __forceinline__ void tma_plane(const CUtensorMap* tm, float* dst, uin
         : "memory");
 }
 
+// the same box, only pulled into L2 (no shared-memory destination, no barrier)
+__device__ __forceinline__ void tma_prefetch_plane(const CUtensorMap* tm, int c0, int c1, int c2, int c3)
+{
+    asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];"
+                 ::"l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
+
 // ---- float4 helpers -----------------------------------------------------------------------------
 __device__ __forceinline__ float4 ld4s(const float* p, int quad) { return *reinterpret_cast<const float4*>(p + 4 * quad); }
 __device__ __forceinline__ float2 ld2s(const float* p, int off) { return *reinterpret_cast<const float2*>(p + off); }
@@ -159,11 +173,30 @@ __device__ __forceinline__ float4 dmx(float2 l, float4 c, float2 r)   // D- : re
 }
 
 __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
+#ifndef FT_LDMODE
+#define FT_LDMODE "nc"
+#endif
+// Predicated 128-bit load INTO the registers of v (no copy of the loaded value, so that the scoreboard
+// wait lands on the first real use, a stage later, and not on a loop-carried register move).
+__device__ __forceinline__ void ldg4_into(float4& v, const float* p, bool pred)
+{
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %5, 0;\n\t"
+        "@p ld.global." FT_LDMODE ".v4.f32 {%0, %1, %2, %3}, [%4];\n\t"
+        "}"
+        : "+f"(v.x), "+f"(v.y), "+f"(v.z), "+f"(v.w)
+        : "l"(p), "r"((int)pred));
+}
 __device__ __forceinline__ void stg4(float* p, float4 v) { *reinterpret_cast<float4*>(p) = v; }
 
 // store the in-grid lanes of a quad starting at column x
 __device__ __forceinline__ void store_quad(float* p, float4 v, int x, int nx)
 {
+#ifdef EXP_NOSTORE
+    if (v.x != 123.456f) return;
+#endif
     if (x + 3 < nx) { stg4(p, v); return; }
     if (x < nx) p[0] = v.x;
     if (x + 1 < nx) p[1] = v.y;
@@ -193,11 +226,15 @@ __device__ __forceinline__ long long idx_x(const FusedArgs& a, int col, int y, i
 __device__ __forceinline__ long long idx_y(const FusedArgs& a, int x, int row, int z) { return ((long long)z * a.wyz + row) * a.nxq + x; }
 __device__ __forceinline__ long long idx_z(const FusedArgs& a, int x, int y, int row) { return ((long long)row * a.ny + y) * a.nxq + x; }
 
-__device__ __forceinline__ float tab1(const float* t, int i, int n) { return (unsigned)i < (unsigned)n ? __ldg(t + i) : 0.0f; }
-// table values at x..x+3 ; 0 outside [0,n) (a = 0: no C-PML term ; b = 0 only ever multiplies zeros there)
-__device__ __forceinline__ float4 tab4(const float* t, int x, int n)
+// The C-PML tables (Eq. 38) of the CTA's x / y window and a ring of z planes are staged in shared
+// memory (zeros outside the grid: a = 0 means no C-PML term ; b = 0 only ever multiplies zeros).
+// Helpers take pointers pre-offset so that t[i] is the value at grid index i (z: t[i & 15]).
+__device__ __forceinline__ float4 tab4(const float* t, int x) { return *reinterpret_cast<const float4*>(t + x); }
+__device__ __forceinline__ void prefetch_l2(const float* p)
 {
-    return make_float4(tab1(t, x, n), tab1(t, x + 1, n), tab1(t, x + 2, n), tab1(t, x + 3, n));
+#ifndef EXP_NOPF
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+#endif
 }
 
 // Forward recursion on the thread's own quad (Eq. 46a / 46c with Eq. 38): m <- b m + a t ; returns t + m
@@ -210,6 +247,26 @@ __device__ __forceinline__ float4 pml_fwd(const float* mi, float* mo, long long 
 __device__ __forceinline__ float4 pml_fwd(const float* mi, float* mo, long long idx, float a1, float b1, float4 t, bool wr)
 {
     const float4 m = fma4(b1, ldg4(mi + idx), a1 * t);
+    if (wr) stg4(mo + idx, m);
+    return t + m;
+}
+
+// same with the old value already in registers (loaded a barrier earlier)
+__device__ __forceinline__ float4 pml_fwd_m(float4 m_old, float* mo, long long idx, float4 a4, float4 b4, float4 t, bool wr)
+{
+    const float4 m = fma4(b4, m_old, a4 * t);
+#ifdef EXP_PMLNOMEM
+    wr = wr && m.x == 123.456f;
+#endif
+    if (wr) stg4(mo + idx, m);
+    return t + m;
+}
+__device__ __forceinline__ float4 pml_fwd_m(float4 m_old, float* mo, long long idx, float a1, float b1, float4 t, bool wr)
+{
+    const float4 m = fma4(b1, m_old, a1 * t);
+#ifdef EXP_PMLNOMEM
+    wr = wr && m.x == 123.456f;
+#endif
     if (wr) stg4(mo + idx, m);
     return t + m;
 }
@@ -229,21 +286,21 @@ __device__ __forceinline__ Taps8 adj_x(const FusedArgs& a, const float* __restri
     const long long row = idx_x(a, 0, y, z);
     int col = xslab_col(a, x);
     if (col >= 0) {
-        const float4 Tn = fma4(tab4(tb, x, a.nx), ldg4(Ti + row + col), c);
+        const float4 Tn = fma4(tab4(tb, x), ldg4(Ti + row + col), c);
         if (wr) stg4(To + row + col, Tn);
-        X.c = tab4(ta, x, a.nx) * Tn;
+        X.c = tab4(ta, x) * Tn;
     }
     col = xslab_col(a, x - 4);
     if (col >= 0) {
         const float4 T = ldg4(Ti + row + col);
-        X.l.x = tab1(ta, x - 2, a.nx) * fmaf(tab1(tb, x - 2, a.nx), T.z, l.x);
-        X.l.y = tab1(ta, x - 1, a.nx) * fmaf(tab1(tb, x - 1, a.nx), T.w, l.y);
+        X.l.x = ta[x - 2] * fmaf(tb[x - 2], T.z, l.x);
+        X.l.y = ta[x - 1] * fmaf(tb[x - 1], T.w, l.y);
     }
     col = xslab_col(a, x + 4);
     if (col >= 0) {
         const float4 T = ldg4(Ti + row + col);
-        X.r.x = tab1(ta, x + 4, a.nx) * fmaf(tab1(tb, x + 4, a.nx), T.x, r.x);
-        X.r.y = tab1(ta, x + 5, a.nx) * fmaf(tab1(tb, x + 5, a.nx), T.y, r.y);
+        X.r.x = ta[x + 4] * fmaf(tb[x + 4], T.x, r.x);
+        X.r.y = ta[x + 5] * fmaf(tb[x + 5], T.y, r.y);
     }
     return X;
 }
@@ -260,9 +317,9 @@ __device__ __forceinline__ float4 adj_y(const FusedArgs& a, const float* __restr
         const int p = yzslab_row(r0 + k, a.ny, a.P);
         if (p >= 0) {
             const long long i = idx_y(a, x, p, z);
-            const float4 Tn = fma4(__ldg(tb + r0 + k), ldg4(Ti + i), s[k]);
+            const float4 Tn = fma4(tb[r0 + k], ldg4(Ti + i), s[k]);
             if (wr && k == own) stg4(To + i, Tn);
-            X[k] = __ldg(ta + r0 + k) * Tn;
+            X[k] = ta[r0 + k] * Tn;
         }
     }
     return d4(X[0], X[1], X[2], X[3]);
@@ -280,9 +337,9 @@ __device__ __forceinline__ float4 adj_z(const FusedArgs& a, const float* __restr
         const int p = yzslab_row(z0 + k, a.nz, a.P);
         if (p >= 0) {
             const long long i = idx_z(a, x, y, p);
-            const float4 Tn = fma4(__ldg(tb + z0 + k), ldg4(Ti + i), s[k]);
+            const float4 Tn = fma4(tb[(z0 + k) & (FT_ZRING - 1)], ldg4(Ti + i), s[k]);
             if (wr && k == own) stg4(To + i, Tn);
-            X[k] = __ldg(ta + z0 + k) * Tn;
+            X[k] = ta[(z0 + k) & (FT_ZRING - 1)] * Tn;
         }
     }
     return d4(X[0], X[1], X[2], X[3]);
@@ -304,6 +361,7 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
     uint64_t* bars = reinterpret_cast<uint64_t*>(sm + FT_OFF_END);
     uint64_t* barG = bars;        // [2]  everything first read by stage 1 of iteration c -> slot c & 1
     uint64_t* barM = bars + 2;    // [3]  mu of plane j -> slot j % 3
+    uint64_t* barU = bars + 5;    // [2]  u_old of plane c, landed in ring slot c % FT_RING -> barrier c & 1
 
     const int tid = threadIdx.x;
     int b = blockIdx.x;
@@ -342,6 +400,17 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
     const float* in = a.in;
     const long long box = a.box;
 
+    if (pml) {   // stage the C-PML tables: x / y windows and the first planes of the z ring (zeros outside the grid)
+        for (int i = tid; i < 4 * FT_TABW; i += FT_NT) {
+            const int t = i / FT_TABW, o = i % FT_TABW - 8;
+            sm[FT_OFF_XT + i] = (unsigned)(x0 + o) < (unsigned)a.nx ? __ldg(a.tab[0][t] + x0 + o) : 0.0f;
+            sm[FT_OFF_YT + i] = (unsigned)(y0 + o) < (unsigned)a.ny ? __ldg(a.tab[1][t] + y0 + o) : 0.0f;
+        }
+        if (tid < 4 * 12) {     // planes zb - 10 .. zb + 1 ; the loop adds plane kk + 3 = zb + 1 + it every iteration
+            const int t = tid / 12, z = zb - 10 + tid % 12;
+            sm[FT_OFF_ZT + t * FT_ZRING + (z & (FT_ZRING - 1))] = (unsigned)z < (unsigned)a.nz ? __ldg(a.tab[2][t] + z) : 0.0f;
+        }
+    }
     if (tid == 0) {
         for (int k = 0; k < 8; ++k) mbar_init(&bars[k], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -379,13 +448,22 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
         tma_plane(&tmM36, sm + FT_OFF_MU + (j % 3) * FT_MPL, bar, cxm, cym, cz0 + j, 1);
     };
 
-    if (tid == 0) { issueG(0); issueG(1); }
+    // u_old(c) lands in the ring slot that u_new(c) will overwrite in place (own quads only)
+    auto issueU = [&](int c) {
+        uint64_t* bar = &barU[c & 1];
+        mbar_expect_tx(bar, 3 * FT_UPL * 4);
+        tma_plane(&tmS36, sm + FT_OFF_UR + (0 * FT_RING + c % FT_RING) * FT_UPL, bar, cx40, cy36, cz0 + c, U1);
+        tma_plane(&tmS36, sm + FT_OFF_UR + (1 * FT_RING + c % FT_RING) * FT_UPL, bar, cx40, cy36, cz0 + c, U2);
+        tma_plane(&tmS36, sm + FT_OFF_UR + (2 * FT_RING + c % FT_RING) * FT_UPL, bar, cx40, cy36, cz0 + c, U3);
+    };
+
+    if (tid == 0) { issueG(0); issueG(1); issueU(0); }
 
     // register windows along z (own column)
     float4 w13a, w13b, w13c;          // s13 at kk-2, kk-1, kk
     float4 w23a, w23b, w23c;          // s23
     float4 w33a, w33b, w33c, w33d;    // s33 at kk-2, kk-1, kk, kk+1
-    float4 uo1, uo2, uo3;             // u_old(kk)
+    float4 u3m2 = f4(0.0f);           // u3(ks-2) of the thread's quad (its ring slot is refilled with u_old by then)
     float4 lam, so11, so22, so12;     // lambda, old s11, s22, s12 at ks = kk - 2
     const float4 z4 = f4(0.0f);
     {
@@ -400,9 +478,6 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
         w33b = ld_ok ? ldg4(in + S33 * box + g - a.sz) : z4;
         w33c = ld_ok ? ldg4(in + S33 * box + g) : z4;
         w33d = ld_ok ? ldg4(in + S33 * box + g + a.sz) : z4;
-        uo1 = ld_ok ? ldg4(in + U1 * box + g) : z4;
-        uo2 = ld_ok ? ldg4(in + U2 * box + g) : z4;
-        uo3 = ld_ok ? ldg4(in + U3 * box + g) : z4;
         lam = so11 = so22 = so12 = z4;
     }
 
@@ -410,10 +485,35 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
     const float kB = 2.0f * a.sgn * PACT_C2, kM = 4.0f * a.sgn * PACT_C2, kL = a.sgn * PACT_C2;
     const float* Rbase = sm + FT_OFF_RHO;
     const float* Abase = sm + FT_OFF_ALP;
-    const float* const* tb = reinterpret_cast<const float* const*>(a.tab);   // tab[3][4] flattened: tb[4 * axis + T_*]
+    // C-PML tables in shared memory, pre-offset: XT(t)[x], YT(t)[y], ZT(t)[z & 15] (t = T_A_INT ..)
+    const float* xt0 = sm + FT_OFF_XT + 8 - x0;
+    const float* yt0 = sm + FT_OFF_YT + 8 - y0;
+    const float* zt0 = sm + FT_OFF_ZT;
+#define XT(t) (xt0 + (t) * FT_TABW)
+#define YT(t) (yt0 + (t) * FT_TABW)
+#define ZT(t) (zt0 + (t) * FT_ZRING)
 
     for (int it = 0; it < itn; ++it) {
         const int kk = zb - 2 + it;
+        // forward C-PML: the nine phi of this thread's quad at plane kk, issued together ahead of the wait
+        // (one exposed latency per stage instead of nine serialised ones)
+        float4 pm[9];
+        if (MODE == FM_FWD) {
+#pragma unroll
+            for (int k = 0; k < 9; ++k) pm[k] = f4(0.0f);
+            if (bx || by || (pml && (kk - 2 < a.P || kk + 2 >= a.nz - 1 - a.P))) {
+                bool ok = pok && (unsigned)kk < (unsigned)a.nz;
+#ifdef EXP_PMLNOMEM
+                ok = false;
+#endif
+                const int pzk = ok ? yzslab_row(kk, a.nz, a.P) : -1;
+                const bool ex = ok && colq >= 0, ey = ok && prow >= 0, ez = pzk >= 0;
+                const long long ix = ex ? idx_x(a, colq, y, kk) : 0, iy = ey ? idx_y(a, x, prow, kk) : 0, iz = ez ? idx_z(a, x, y, pzk) : 0;
+                ldg4_into(pm[0], a.mvi[0] + ix, ex); ldg4_into(pm[3], a.mvi[3] + ix, ex); ldg4_into(pm[6], a.mvi[6] + ix, ex);
+                ldg4_into(pm[1], a.mvi[1] + iy, ey); ldg4_into(pm[4], a.mvi[4] + iy, ey); ldg4_into(pm[7], a.mvi[7] + iy, ey);
+                ldg4_into(pm[2], a.mvi[2] + iz, ez); ldg4_into(pm[5], a.mvi[5] + iz, ez); ldg4_into(pm[8], a.mvi[8] + iz, ez);
+            }
+        }
         mbar_wait(&barG[it & 1], (it >> 1) & 1);
 
         const int s3 = it % 3, s3n = (it + 1) % 3;
@@ -438,62 +538,89 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
             const bool bz = pml && (kk - 2 < a.P || kk + 2 >= a.nz - 1 - a.P);
             const bool pml1 = (bx || by || bz) && pok && zin;
 
+            if (pml && pok && (unsigned)(kk + 2) < (unsigned)a.nz) {
+                // pull the memory variables of plane kk + 2 into L2 (there is no L1 left beside 227 KB of shared memory)
+                const int zp = kk + 2;
+                const bool psi = MODE == FM_ADJ || inner;      // forward: psi is only touched by the owner
+                if (colq >= 0) {
+                    const long long i = idx_x(a, colq, y, zp);
+                    prefetch_l2(a.mvi[0] + i); prefetch_l2(a.mvi[3] + i); prefetch_l2(a.mvi[6] + i);
+                    if (psi) { prefetch_l2(a.mvi[9] + i); prefetch_l2(a.mvi[12] + i); prefetch_l2(a.mvi[15] + i); }
+                }
+                if (prow >= 0) {
+                    const long long i = idx_y(a, x, prow, zp);
+                    prefetch_l2(a.mvi[1] + i); prefetch_l2(a.mvi[4] + i); prefetch_l2(a.mvi[7] + i);
+                    if (psi) { prefetch_l2(a.mvi[10] + i); prefetch_l2(a.mvi[13] + i); prefetch_l2(a.mvi[16] + i); }
+                }
+                const int pzp = yzslab_row(zp, a.nz, a.P);
+                if (pzp >= 0) {
+                    const long long i = idx_z(a, x, y, pzp);
+                    prefetch_l2(a.mvi[2] + i); prefetch_l2(a.mvi[5] + i); prefetch_l2(a.mvi[8] + i);
+                    if (psi) { prefetch_l2(a.mvi[11] + i); prefetch_l2(a.mvi[14] + i); prefetch_l2(a.mvi[17] + i); }
+                }
+            }
+
             // staggered coefficients (reading G10): J = 1 - dt alpha_b, B = dt/(h rho_b)
             const float4 r0 = ld4s(PR, q), a0 = ld4s(PA, q);
             const float4 one = f4(1.0f), mh = f4(-0.5f);
             const float4 c12 = ld4s(P12, q);
             float4 n1, n2, n3;
+            const int sl = it % FT_RING;
+            float* const R1 = sm + FT_OFF_UR + (0 * FT_RING + sl) * FT_UPL + 4 * uq;
+            float* const R2 = sm + FT_OFF_UR + (1 * FT_RING + sl) * FT_UPL + 4 * uq;
+            float* const R3 = sm + FT_OFF_UR + (2 * FT_RING + sl) * FT_UPL + 4 * uq;
             {   // ---- u1 at (x+1/2, y, z): D+x s11, D-y s12, D-z s13
                 const float4 c11 = ld4s(P11, q);
                 const float2 l = ld2s(P11, 4 * q - 2), rr = ld2s(P11, 4 * q + 4);
                 const float4 ya = ld4s(P12, q - 20), yb = ld4s(P12, q - 10), yd = ld4s(P12, q + 10);
                 float4 t1 = dpx(l, c11, rr), t2 = d4(ya, yb, c12, yd), t3 = d4(w13a, w13b, w13c, f13);
                 if (MODE == FM_FWD && pml1) {
-                    if (colq >= 0) t1 = pml_fwd(a.mvi[0], a.mvo[0], idx_x(a, colq, y, kk), tab4(tb[T_A_HALF], x, a.nx), tab4(tb[T_B_HALF], x, a.nx), t1, wr1);
-                    if (prow >= 0) t2 = pml_fwd(a.mvi[1], a.mvo[1], idx_y(a, x, prow, kk), __ldg(tb[4 + T_A_INT] + y), __ldg(tb[4 + T_B_INT] + y), t2, wr1);
-                    if (pz >= 0) t3 = pml_fwd(a.mvi[2], a.mvo[2], idx_z(a, x, y, pz), __ldg(tb[8 + T_A_INT] + kk), __ldg(tb[8 + T_B_INT] + kk), t3, wr1);
+                    if (colq >= 0) t1 = pml_fwd_m(pm[0], a.mvo[0], idx_x(a, colq, y, kk), tab4(XT(T_A_HALF), x), tab4(XT(T_B_HALF), x), t1, wr1);
+                    if (prow >= 0) t2 = pml_fwd_m(pm[1], a.mvo[1], idx_y(a, x, prow, kk), YT(T_A_INT)[y], YT(T_B_INT)[y], t2, wr1);
+                    if (pz >= 0) t3 = pml_fwd_m(pm[2], a.mvo[2], idx_z(a, x, y, pz), ZT(T_A_INT)[kk & (FT_ZRING - 1)], ZT(T_B_INT)[kk & (FT_ZRING - 1)], t3, wr1);
                 }
                 if (MODE == FM_ADJ && pml1) {
-                    if (bx) { const Taps8 X = adj_x(a, a.mvi[9], a.mvo[9], tb[T_A_INT], tb[T_B_INT], x, y, kk, l, c11, rr, wr1); t1 = t1 + dpx(X.l, X.c, X.r); }
-                    if (by) t2 = t2 + adj_y(a, a.mvi[10], a.mvo[10], tb[4 + T_A_HALF], tb[4 + T_B_HALF], x, y - 2, kk, 2, ya, yb, c12, yd, wr1);
-                    if (bz) t3 = t3 + adj_z(a, a.mvi[11], a.mvo[11], tb[8 + T_A_HALF], tb[8 + T_B_HALF], x, y, kk - 2, 2, w13a, w13b, w13c, f13, wr1);
+                    if (bx) { const Taps8 X = adj_x(a, a.mvi[9], a.mvo[9], XT(T_A_INT), XT(T_B_INT), x, y, kk, l, c11, rr, wr1); t1 = t1 + dpx(X.l, X.c, X.r); }
+                    if (by) t2 = t2 + adj_y(a, a.mvi[10], a.mvo[10], YT(T_A_HALF), YT(T_B_HALF), x, y - 2, kk, 2, ya, yb, c12, yd, wr1);
+                    if (bz) t3 = t3 + adj_z(a, a.mvi[11], a.mvo[11], ZT(T_A_HALF), ZT(T_B_HALF), x, y, kk - 2, 2, w13a, w13b, w13c, f13, wr1);
                 }
                 const float4 rxp = shl1(r0, PR[4 * q + 4]), axp = shl1(a0, PA[4 * q + 4]);
-                n1 = fma4(fma4(mh, a0 + axp, one), uo1, (kB * rcp4(r0 + rxp)) * (t1 + t2 + t3));
+                mbar_wait(&barU[it & 1], (it >> 1) & 1);      // u_old(kk) has landed in the ring slot
+                n1 = fma4(fma4(mh, a0 + axp, one), *reinterpret_cast<const float4*>(R1), (kB * rcp4(r0 + rxp)) * (t1 + t2 + t3));
             }
             {   // ---- u2 at (x, y+1/2, z): D-x s12, D+y s22, D-z s23
                 const float2 l = ld2s(P12, 4 * q - 2), rr = ld2s(P12, 4 * q + 4);
                 const float4 yb = ld4s(P22, q - 10), c22 = ld4s(P22, q), yc = ld4s(P22, q + 10), yd = ld4s(P22, q + 20);
                 float4 t1 = dmx(l, c12, rr), t2 = d4(yb, c22, yc, yd), t3 = d4(w23a, w23b, w23c, f23);
                 if (MODE == FM_FWD && pml1) {
-                    if (colq >= 0) t1 = pml_fwd(a.mvi[3], a.mvo[3], idx_x(a, colq, y, kk), tab4(tb[T_A_INT], x, a.nx), tab4(tb[T_B_INT], x, a.nx), t1, wr1);
-                    if (prow >= 0) t2 = pml_fwd(a.mvi[4], a.mvo[4], idx_y(a, x, prow, kk), __ldg(tb[4 + T_A_HALF] + y), __ldg(tb[4 + T_B_HALF] + y), t2, wr1);
-                    if (pz >= 0) t3 = pml_fwd(a.mvi[5], a.mvo[5], idx_z(a, x, y, pz), __ldg(tb[8 + T_A_INT] + kk), __ldg(tb[8 + T_B_INT] + kk), t3, wr1);
+                    if (colq >= 0) t1 = pml_fwd_m(pm[3], a.mvo[3], idx_x(a, colq, y, kk), tab4(XT(T_A_INT), x), tab4(XT(T_B_INT), x), t1, wr1);
+                    if (prow >= 0) t2 = pml_fwd_m(pm[4], a.mvo[4], idx_y(a, x, prow, kk), YT(T_A_HALF)[y], YT(T_B_HALF)[y], t2, wr1);
+                    if (pz >= 0) t3 = pml_fwd_m(pm[5], a.mvo[5], idx_z(a, x, y, pz), ZT(T_A_INT)[kk & (FT_ZRING - 1)], ZT(T_B_INT)[kk & (FT_ZRING - 1)], t3, wr1);
                 }
                 if (MODE == FM_ADJ && pml1) {
-                    if (bx) { const Taps8 X = adj_x(a, a.mvi[12], a.mvo[12], tb[T_A_HALF], tb[T_B_HALF], x, y, kk, l, c12, rr, wr1); t1 = t1 + dmx(X.l, X.c, X.r); }
-                    if (by) t2 = t2 + adj_y(a, a.mvi[13], a.mvo[13], tb[4 + T_A_INT], tb[4 + T_B_INT], x, y - 1, kk, 1, yb, c22, yc, yd, wr1);
-                    if (bz) t3 = t3 + adj_z(a, a.mvi[14], a.mvo[14], tb[8 + T_A_HALF], tb[8 + T_B_HALF], x, y, kk - 2, 2, w23a, w23b, w23c, f23, wr1);
+                    if (bx) { const Taps8 X = adj_x(a, a.mvi[12], a.mvo[12], XT(T_A_HALF), XT(T_B_HALF), x, y, kk, l, c12, rr, wr1); t1 = t1 + dmx(X.l, X.c, X.r); }
+                    if (by) t2 = t2 + adj_y(a, a.mvi[13], a.mvo[13], YT(T_A_INT), YT(T_B_INT), x, y - 1, kk, 1, yb, c22, yc, yd, wr1);
+                    if (bz) t3 = t3 + adj_z(a, a.mvi[14], a.mvo[14], ZT(T_A_HALF), ZT(T_B_HALF), x, y, kk - 2, 2, w23a, w23b, w23c, f23, wr1);
                 }
                 const float4 ryp = ld4s(PR, q + 10), ayp = ld4s(PA, q + 10);
-                n2 = fma4(fma4(mh, a0 + ayp, one), uo2, (kB * rcp4(r0 + ryp)) * (t1 + t2 + t3));
+                n2 = fma4(fma4(mh, a0 + ayp, one), *reinterpret_cast<const float4*>(R2), (kB * rcp4(r0 + ryp)) * (t1 + t2 + t3));
             }
             {   // ---- u3 at (x, y, z+1/2): D-x s13, D-y s23, D+z s33
                 const float2 l = ld2s(P13, 4 * q - 2), rr = ld2s(P13, 4 * q + 4);
                 const float4 ya = ld4s(P23, q - 20), yb = ld4s(P23, q - 10), yd = ld4s(P23, q + 10);
                 float4 t1 = dmx(l, w13c, rr), t2 = d4(ya, yb, w23c, yd), t3 = d4(w33b, w33c, w33d, f33);
                 if (MODE == FM_FWD && pml1) {
-                    if (colq >= 0) t1 = pml_fwd(a.mvi[6], a.mvo[6], idx_x(a, colq, y, kk), tab4(tb[T_A_INT], x, a.nx), tab4(tb[T_B_INT], x, a.nx), t1, wr1);
-                    if (prow >= 0) t2 = pml_fwd(a.mvi[7], a.mvo[7], idx_y(a, x, prow, kk), __ldg(tb[4 + T_A_INT] + y), __ldg(tb[4 + T_B_INT] + y), t2, wr1);
-                    if (pz >= 0) t3 = pml_fwd(a.mvi[8], a.mvo[8], idx_z(a, x, y, pz), __ldg(tb[8 + T_A_HALF] + kk), __ldg(tb[8 + T_B_HALF] + kk), t3, wr1);
+                    if (colq >= 0) t1 = pml_fwd_m(pm[6], a.mvo[6], idx_x(a, colq, y, kk), tab4(XT(T_A_INT), x), tab4(XT(T_B_INT), x), t1, wr1);
+                    if (prow >= 0) t2 = pml_fwd_m(pm[7], a.mvo[7], idx_y(a, x, prow, kk), YT(T_A_INT)[y], YT(T_B_INT)[y], t2, wr1);
+                    if (pz >= 0) t3 = pml_fwd_m(pm[8], a.mvo[8], idx_z(a, x, y, pz), ZT(T_A_HALF)[kk & (FT_ZRING - 1)], ZT(T_B_HALF)[kk & (FT_ZRING - 1)], t3, wr1);
                 }
                 if (MODE == FM_ADJ && pml1) {
-                    if (bx) { const Taps8 X = adj_x(a, a.mvi[15], a.mvo[15], tb[T_A_HALF], tb[T_B_HALF], x, y, kk, l, w13c, rr, wr1); t1 = t1 + dmx(X.l, X.c, X.r); }
-                    if (by) t2 = t2 + adj_y(a, a.mvi[16], a.mvo[16], tb[4 + T_A_HALF], tb[4 + T_B_HALF], x, y - 2, kk, 2, ya, yb, w23c, yd, wr1);
-                    if (bz) t3 = t3 + adj_z(a, a.mvi[17], a.mvo[17], tb[8 + T_A_INT], tb[8 + T_B_INT], x, y, kk - 1, 1, w33b, w33c, w33d, f33, wr1);
+                    if (bx) { const Taps8 X = adj_x(a, a.mvi[15], a.mvo[15], XT(T_A_HALF), XT(T_B_HALF), x, y, kk, l, w13c, rr, wr1); t1 = t1 + dmx(X.l, X.c, X.r); }
+                    if (by) t2 = t2 + adj_y(a, a.mvi[16], a.mvo[16], YT(T_A_HALF), YT(T_B_HALF), x, y - 2, kk, 2, ya, yb, w23c, yd, wr1);
+                    if (bz) t3 = t3 + adj_z(a, a.mvi[17], a.mvo[17], ZT(T_A_INT), ZT(T_B_INT), x, y, kk - 1, 1, w33b, w33c, w33d, f33, wr1);
                 }
                 const float4 rzp = ld4s(Rbase + s3n * FT_BOX, q), azp = ld4s(Abase + s3n * FT_BOX, q);
-                n3 = fma4(fma4(mh, a0 + azp, one), uo3, (kB * rcp4(r0 + rzp)) * (t1 + t2 + t3));
+                n3 = fma4(fma4(mh, a0 + azp, one), *reinterpret_cast<const float4*>(R3), (kB * rcp4(r0 + rzp)) * (t1 + t2 + t3));
             }
             if (edge_xy || !zin) {
                 if (!(zin && m0)) { n1.x = 0.0f; n2.x = 0.0f; n3.x = 0.0f; }
@@ -501,10 +628,9 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                 if (!(zin && m2)) { n1.z = 0.0f; n2.z = 0.0f; n3.z = 0.0f; }
                 if (!(zin && m3)) { n1.w = 0.0f; n2.w = 0.0f; n3.w = 0.0f; }
             }
-            const int sl = it % FT_RING;
-            *reinterpret_cast<float4*>(sm + FT_OFF_UR + (0 * FT_RING + sl) * FT_UPL + 4 * uq) = n1;
-            *reinterpret_cast<float4*>(sm + FT_OFF_UR + (1 * FT_RING + sl) * FT_UPL + 4 * uq) = n2;
-            *reinterpret_cast<float4*>(sm + FT_OFF_UR + (2 * FT_RING + sl) * FT_UPL + 4 * uq) = n3;
+            *reinterpret_cast<float4*>(R1) = n1;
+            *reinterpret_cast<float4*>(R2) = n2;
+            *reinterpret_cast<float4*>(R3) = n3;
             const long long g = (long long)kk * a.sz + gxy;
             if (wr1) {
                 store_quad(a.out + U1 * box + g, n1, x, a.nx);
@@ -513,43 +639,63 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                 if (MODE == FM_ADJ && pml1) {   // phi_bar (tilde form) fed by the new u_bar: Eq. 61c,e in scaled variables
                     if (colq >= 0) {
                         const long long i = idx_x(a, colq, y, kk);
-                        const float4 bi = tab4(tb[T_B_INT], x, a.nx);
-                        adj_own(a.mvi[0], a.mvo[0], i, tab4(tb[T_B_HALF], x, a.nx), n1);
+                        const float4 bi = tab4(XT(T_B_INT), x);
+                        adj_own(a.mvi[0], a.mvo[0], i, tab4(XT(T_B_HALF), x), n1);
                         adj_own(a.mvi[3], a.mvo[3], i, bi, n2);
                         adj_own(a.mvi[6], a.mvo[6], i, bi, n3);
                     }
                     if (prow >= 0) {
                         const long long i = idx_y(a, x, prow, kk);
-                        const float bi = __ldg(tb[4 + T_B_INT] + y);
+                        const float bi = YT(T_B_INT)[y];
                         adj_own(a.mvi[1], a.mvo[1], i, bi, n1);
-                        adj_own(a.mvi[4], a.mvo[4], i, __ldg(tb[4 + T_B_HALF] + y), n2);
+                        adj_own(a.mvi[4], a.mvo[4], i, YT(T_B_HALF)[y], n2);
                         adj_own(a.mvi[7], a.mvo[7], i, bi, n3);
                     }
                     if (pz >= 0) {
                         const long long i = idx_z(a, x, y, pz);
-                        const float bi = __ldg(tb[8 + T_B_INT] + kk);
+                        const float bi = ZT(T_B_INT)[kk & (FT_ZRING - 1)];
                         adj_own(a.mvi[2], a.mvo[2], i, bi, n1);
                         adj_own(a.mvi[5], a.mvo[5], i, bi, n2);
-                        adj_own(a.mvi[8], a.mvo[8], i, __ldg(tb[8 + T_B_HALF] + kk), n3);
+                        adj_own(a.mvi[8], a.mvo[8], i, ZT(T_B_HALF)[kk & (FT_ZRING - 1)], n3);
                     }
                 }
             }
-            // u_old of the next plane (in flight during stage 2)
-            if (ld_ok && it + 1 < itn) {
-                uo1 = ldg4(in + U1 * box + g + a.sz);
-                uo2 = ldg4(in + U2 * box + g + a.sz);
-                uo3 = ldg4(in + U3 * box + g + a.sz);
+        }
+        // forward C-PML: the nine psi of the quad at plane ks = kk - 2, issued ahead of the barrier
+        float4 qm[9];
+        if (MODE == FM_FWD) {
+#pragma unroll
+            for (int k = 0; k < 9; ++k) qm[k] = f4(0.0f);
+            if (bx || by || (pml && (kk - 4 < a.P || kk >= a.nz - 1 - a.P))) {
+                bool ok = inner && it >= 4;
+#ifdef EXP_PMLNOMEM
+                ok = false;
+#endif
+                const int pzk = ok ? yzslab_row(kk - 2, a.nz, a.P) : -1;
+                const bool ex = ok && colq >= 0, ey = ok && prow >= 0, ez = pzk >= 0;
+                const long long ix = ex ? idx_x(a, colq, y, kk - 2) : 0, iy = ey ? idx_y(a, x, prow, kk - 2) : 0, iz = ez ? idx_z(a, x, y, pzk) : 0;
+                ldg4_into(qm[0], a.mvi[9] + ix, ex); ldg4_into(qm[3], a.mvi[12] + ix, ex); ldg4_into(qm[6], a.mvi[15] + ix, ex);
+                ldg4_into(qm[1], a.mvi[10] + iy, ey); ldg4_into(qm[4], a.mvi[13] + iy, ey); ldg4_into(qm[7], a.mvi[16] + iy, ey);
+                ldg4_into(qm[2], a.mvi[11] + iz, ez); ldg4_into(qm[5], a.mvi[14] + iz, ez); ldg4_into(qm[8], a.mvi[17] + iz, ez);
             }
+        }
+        if (pml && tid >= 360 && tid < 364) {   // z table ring: plane kk + 3 (first read after the barrier)
+            const int t = tid - 360, z = kk + 3;
+            sm[FT_OFF_ZT + t * FT_ZRING + (z & (FT_ZRING - 1))] = (unsigned)z < (unsigned)a.nz ? __ldg(a.tab[2][t] + z) : 0.0f;
         }
         __syncthreads();
         // every thread is past stage 1 of `it` and stage 2 of `it - 1`: refill the slots they freed
         if (tid == 0) {
             if (it + 2 < itn) issueG(it + 2);
-            if (it + 2 <= itn) issueM(it);   // mu(j) is read by stage 2 of iterations j + 1 and j + 2
+            if (it + 2 <= itn) issueM(it);
+            if (it + 1 < itn) issueU(it + 1);   // slot of plane it - 4: its last cross-thread reads were in stage 2 of it - 2
         }
         if (it >= 1) mbar_wait(&barM[(it - 1) % 3], ((it - 1) / 3) & 1);
         // ------------------------------------------------------------------ stage 2: sigma(ks), ks = kk - 2
         const int ks = kk - 2;
+        // u3(ks-1) of the own quad; with u3m2 (the value read here one iteration ago) it replaces the two oldest ring planes
+        float4 u3m1 = z4;
+        if (inner && it >= 3) u3m1 = ld4s(sm + FT_OFF_UR + (2 * FT_RING + (it + 2) % FT_RING) * FT_UPL, uq);
         if (inner && it >= 4) {
             const int j = it - 2;             // relative plane of ks
             const float* U1p = sm + FT_OFF_UR + 0 * FT_RING * FT_UPL;
@@ -568,14 +714,14 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                 const float4 za = ld4s(U1p + pm1, uq), zc = ld4s(U1p + pp1, uq), zd = ld4s(U1p + pp2, uq);
                 e11 = dmx(l, c, rr); g12 = d4(ya, c, yc, yd); g13 = d4(za, c, zc, zd);
                 if (MODE == FM_FWD && pml2) {
-                    if (colq >= 0) e11 = pml_fwd(a.mvi[9], a.mvo[9], idx_x(a, colq, y, ks), tab4(tb[T_A_INT], x, a.nx), tab4(tb[T_B_INT], x, a.nx), e11, true);
-                    if (prow >= 0) g12 = pml_fwd(a.mvi[10], a.mvo[10], idx_y(a, x, prow, ks), __ldg(tb[4 + T_A_HALF] + y), __ldg(tb[4 + T_B_HALF] + y), g12, true);
-                    if (pz >= 0) g13 = pml_fwd(a.mvi[11], a.mvo[11], idx_z(a, x, y, pz), __ldg(tb[8 + T_A_HALF] + ks), __ldg(tb[8 + T_B_HALF] + ks), g13, true);
+                    if (colq >= 0) e11 = pml_fwd_m(qm[0], a.mvo[9], idx_x(a, colq, y, ks), tab4(XT(T_A_INT), x), tab4(XT(T_B_INT), x), e11, true);
+                    if (prow >= 0) g12 = pml_fwd_m(qm[1], a.mvo[10], idx_y(a, x, prow, ks), YT(T_A_HALF)[y], YT(T_B_HALF)[y], g12, true);
+                    if (pz >= 0) g13 = pml_fwd_m(qm[2], a.mvo[11], idx_z(a, x, y, pz), ZT(T_A_HALF)[ks & (FT_ZRING - 1)], ZT(T_B_HALF)[ks & (FT_ZRING - 1)], g13, true);
                 }
                 if (MODE == FM_ADJ && pml2) {
-                    if (bx) { const Taps8 X = adj_x(a, a.mvi[0], nullptr, tb[T_A_HALF], tb[T_B_HALF], x, y, ks, l, c, rr, false); e11 = e11 + dmx(X.l, X.c, X.r); }
-                    if (by) g12 = g12 + adj_y(a, a.mvi[1], nullptr, tb[4 + T_A_INT], tb[4 + T_B_INT], x, y - 1, ks, 1, ya, c, yc, yd, false);
-                    if (bz) g13 = g13 + adj_z(a, a.mvi[2], nullptr, tb[8 + T_A_INT], tb[8 + T_B_INT], x, y, ks - 1, 1, za, c, zc, zd, false);
+                    if (bx) { const Taps8 X = adj_x(a, a.mvi[0], nullptr, XT(T_A_HALF), XT(T_B_HALF), x, y, ks, l, c, rr, false); e11 = e11 + dmx(X.l, X.c, X.r); }
+                    if (by) g12 = g12 + adj_y(a, a.mvi[1], nullptr, YT(T_A_INT), YT(T_B_INT), x, y - 1, ks, 1, ya, c, yc, yd, false);
+                    if (bz) g13 = g13 + adj_z(a, a.mvi[2], nullptr, ZT(T_A_INT), ZT(T_B_INT), x, y, ks - 1, 1, za, c, zc, zd, false);
                 }
             }
             {   // ---- derivatives of u2: D+x (g21), D-y (e22), D+z (g23)
@@ -585,31 +731,31 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                 const float4 za = ld4s(U2p + pm1, uq), zc = ld4s(U2p + pp1, uq), zd = ld4s(U2p + pp2, uq);
                 g21 = dpx(l, c, rr); e22 = d4(ya, yb, c, yd); g23 = d4(za, c, zc, zd);
                 if (MODE == FM_FWD && pml2) {
-                    if (colq >= 0) g21 = pml_fwd(a.mvi[12], a.mvo[12], idx_x(a, colq, y, ks), tab4(tb[T_A_HALF], x, a.nx), tab4(tb[T_B_HALF], x, a.nx), g21, true);
-                    if (prow >= 0) e22 = pml_fwd(a.mvi[13], a.mvo[13], idx_y(a, x, prow, ks), __ldg(tb[4 + T_A_INT] + y), __ldg(tb[4 + T_B_INT] + y), e22, true);
-                    if (pz >= 0) g23 = pml_fwd(a.mvi[14], a.mvo[14], idx_z(a, x, y, pz), __ldg(tb[8 + T_A_HALF] + ks), __ldg(tb[8 + T_B_HALF] + ks), g23, true);
+                    if (colq >= 0) g21 = pml_fwd_m(qm[3], a.mvo[12], idx_x(a, colq, y, ks), tab4(XT(T_A_HALF), x), tab4(XT(T_B_HALF), x), g21, true);
+                    if (prow >= 0) e22 = pml_fwd_m(qm[4], a.mvo[13], idx_y(a, x, prow, ks), YT(T_A_INT)[y], YT(T_B_INT)[y], e22, true);
+                    if (pz >= 0) g23 = pml_fwd_m(qm[5], a.mvo[14], idx_z(a, x, y, pz), ZT(T_A_HALF)[ks & (FT_ZRING - 1)], ZT(T_B_HALF)[ks & (FT_ZRING - 1)], g23, true);
                 }
                 if (MODE == FM_ADJ && pml2) {
-                    if (bx) { const Taps8 X = adj_x(a, a.mvi[3], nullptr, tb[T_A_INT], tb[T_B_INT], x, y, ks, l, c, rr, false); g21 = g21 + dpx(X.l, X.c, X.r); }
-                    if (by) e22 = e22 + adj_y(a, a.mvi[4], nullptr, tb[4 + T_A_HALF], tb[4 + T_B_HALF], x, y - 2, ks, 2, ya, yb, c, yd, false);
-                    if (bz) g23 = g23 + adj_z(a, a.mvi[5], nullptr, tb[8 + T_A_INT], tb[8 + T_B_INT], x, y, ks - 1, 1, za, c, zc, zd, false);
+                    if (bx) { const Taps8 X = adj_x(a, a.mvi[3], nullptr, XT(T_A_INT), XT(T_B_INT), x, y, ks, l, c, rr, false); g21 = g21 + dpx(X.l, X.c, X.r); }
+                    if (by) e22 = e22 + adj_y(a, a.mvi[4], nullptr, YT(T_A_HALF), YT(T_B_HALF), x, y - 2, ks, 2, ya, yb, c, yd, false);
+                    if (bz) g23 = g23 + adj_z(a, a.mvi[5], nullptr, ZT(T_A_INT), ZT(T_B_INT), x, y, ks - 1, 1, za, c, zc, zd, false);
                 }
             }
             {   // ---- derivatives of u3: D+x (g31), D+y (g32), D-z (e33)
                 const float4 c = ld4s(U3p + p0, uq);
                 const float2 l = ld2s(U3p + p0, 4 * uq - 2), rr = ld2s(U3p + p0, 4 * uq + 4);
                 const float4 ya = ld4s(U3p + p0, uq - 10), yc = ld4s(U3p + p0, uq + 10), yd = ld4s(U3p + p0, uq + 20);
-                const float4 za = ld4s(U3p + pm2, uq), zb_ = ld4s(U3p + pm1, uq), zd = ld4s(U3p + pp1, uq);
+                const float4 za = u3m2, zb_ = u3m1, zd = ld4s(U3p + pp1, uq);
                 g31 = dpx(l, c, rr); g32 = d4(ya, c, yc, yd); e33 = d4(za, zb_, c, zd);
                 if (MODE == FM_FWD && pml2) {
-                    if (colq >= 0) g31 = pml_fwd(a.mvi[15], a.mvo[15], idx_x(a, colq, y, ks), tab4(tb[T_A_HALF], x, a.nx), tab4(tb[T_B_HALF], x, a.nx), g31, true);
-                    if (prow >= 0) g32 = pml_fwd(a.mvi[16], a.mvo[16], idx_y(a, x, prow, ks), __ldg(tb[4 + T_A_HALF] + y), __ldg(tb[4 + T_B_HALF] + y), g32, true);
-                    if (pz >= 0) e33 = pml_fwd(a.mvi[17], a.mvo[17], idx_z(a, x, y, pz), __ldg(tb[8 + T_A_INT] + ks), __ldg(tb[8 + T_B_INT] + ks), e33, true);
+                    if (colq >= 0) g31 = pml_fwd_m(qm[6], a.mvo[15], idx_x(a, colq, y, ks), tab4(XT(T_A_HALF), x), tab4(XT(T_B_HALF), x), g31, true);
+                    if (prow >= 0) g32 = pml_fwd_m(qm[7], a.mvo[16], idx_y(a, x, prow, ks), YT(T_A_HALF)[y], YT(T_B_HALF)[y], g32, true);
+                    if (pz >= 0) e33 = pml_fwd_m(qm[8], a.mvo[17], idx_z(a, x, y, pz), ZT(T_A_INT)[ks & (FT_ZRING - 1)], ZT(T_B_INT)[ks & (FT_ZRING - 1)], e33, true);
                 }
                 if (MODE == FM_ADJ && pml2) {
-                    if (bx) { const Taps8 X = adj_x(a, a.mvi[6], nullptr, tb[T_A_INT], tb[T_B_INT], x, y, ks, l, c, rr, false); g31 = g31 + dpx(X.l, X.c, X.r); }
-                    if (by) g32 = g32 + adj_y(a, a.mvi[7], nullptr, tb[4 + T_A_INT], tb[4 + T_B_INT], x, y - 1, ks, 1, ya, c, yc, yd, false);
-                    if (bz) e33 = e33 + adj_z(a, a.mvi[8], nullptr, tb[8 + T_A_HALF], tb[8 + T_B_HALF], x, y, ks - 2, 2, za, zb_, c, zd, false);
+                    if (bx) { const Taps8 X = adj_x(a, a.mvi[6], nullptr, XT(T_A_INT), XT(T_B_INT), x, y, ks, l, c, rr, false); g31 = g31 + dpx(X.l, X.c, X.r); }
+                    if (by) g32 = g32 + adj_y(a, a.mvi[7], nullptr, YT(T_A_INT), YT(T_B_INT), x, y - 1, ks, 1, ya, c, yc, yd, false);
+                    if (bz) e33 = e33 + adj_z(a, a.mvi[8], nullptr, ZT(T_A_HALF), ZT(T_B_HALF), x, y, ks - 2, 2, za, zb_, c, zd, false);
                 }
             }
 
@@ -637,13 +783,15 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
             store_quad(a.out + S13 * box + g, n13, x, a.nx);
             store_quad(a.out + S23 * box + g, n23, x, a.nx);
         }
-        if (inner && it >= 3 && it + 1 < itn) {   // own-column inputs of the next stage 2 (plane ks + 1)
+        {   // own-column inputs of the next stage 2 (plane ks + 1)
+            const bool p = inner && it >= 3 && it + 1 < itn;
             const long long g = (long long)(ks + 1) * a.sz + gxy;
-            lam = ldg4(a.mat + g);
-            so11 = ldg4(in + S11 * box + g);
-            so22 = ldg4(in + S22 * box + g);
-            so12 = ldg4(in + S12 * box + g);
+            ldg4_into(lam, a.mat + g, p);
+            ldg4_into(so11, in + S11 * box + g, p);
+            ldg4_into(so22, in + S22 * box + g, p);
+            ldg4_into(so12, in + S12 * box + g, p);
         }
+        u3m2 = u3m1;
         // slide the z windows
         w13a = w13b; w13b = w13c; w13c = f13;
         w23a = w23b; w23b = w23c; w23c = f23;
