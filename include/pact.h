@@ -106,8 +106,10 @@ const char* pact_last_cuda_error(void);
  *   "profile"  1: record CUDA events on the context's stream around the time loop and around
  *              sampled kernel launches of the next pact_forward/pact_adjoint; read them with
  *              pact_get_timing.  0 (default): no events.
- *   "variant"  step-kernel implementation: 0 = default (best available), 1 = plain two-kernel
- *              in-place path, 2 = fused single-pass path.
+ *   "variant"  step-kernel implementation: 0 = automatic (fused when the grid has at least one
+ *              32 x 32 x 32 brick per SM, else plain), 1 = plain two-kernel in-place path, 2 = fused
+ *              single-pass path (TMA-staged z-marching kernel, two state buffers).  A medium with
+ *              3 lambda + 2 mu <= 0 somewhere always takes the plain path.
  *   "graph"    1: replay the time loop from a captured CUDA graph (default for small grids);
  *              0: launch directly; -1: automatic.
  *   "zchunk"   planes of z each CTA of the fused kernel marches over (0 = automatic).  Any value

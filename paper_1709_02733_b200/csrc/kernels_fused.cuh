@@ -10,9 +10,10 @@
 //   stage 1 (Eq. 46a,b): u(kk) on the tile + 2 cells of ring, from sigma on the tile + 4 cells;
 //   stage 2 (Eq. 46c,d): sigma(kk-2) on the tile, from u(kk-4 .. kk) kept in a shared-memory ring.
 // Fields whose x/y neighbours are needed (s11,s22,s12,s13,s23, rho, alpha, mu) and s33 arrive in
-// shared memory by TMA (cp.async.bulk.tensor, mbarrier complete_tx), two planes ahead of use; the
-// z neighbours of s13,s23,s33 live in per-thread register windows; u_old, lambda and the old
-// s11,s22,s12 are own-column values fetched with 128-bit loads one stage ahead of use.
+// shared memory by TMA (cp.async.bulk.tensor, mbarrier complete_tx), two planes ahead of use; u_old(kk)
+// lands by TMA in the very ring slot that u_new(kk) then overwrites in place; the z neighbours of
+// s13,s23,s33 (and the oldest u3 tap) live in per-thread registers; lambda and the old s11,s22,s12
+// of stage 2 are own-column 128-bit loads issued one stage ahead of use (L2 hits but for lambda).
 // The ring of 2 (4) cells around the tile is recomputed by the neighbouring CTAs; nothing is
 // exchanged between CTAs, hence the two state buffers.
 //
@@ -40,9 +41,7 @@
 #define FT_MW 36                      // mu box: tile + 1 (rounded up to a quad) in x
 #define FT_MH 33                      //         tile + 1 in y
 #define FT_MPL 1216                   // floats per mu plane buffer (36*33 = 1188, padded to 128 B)
-#ifndef FT_RING
-#define FT_RING 5                     // u planes kept for stage 2: ks-2 .. ks+2
-#endif
+#define FT_RING 5                     // u planes in the ring: ks-1 .. ks+2 and the slot u_old(kk+1) is landing in
 
 // shared memory map (floats)
 #define FT_OFF_S11 0
@@ -173,9 +172,6 @@ __device__ __forceinline__ float4 dmx(float2 l, float4 c, float2 r)   // D- : re
 }
 
 __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
-#ifndef FT_LDMODE
-#define FT_LDMODE "nc"
-#endif
 // Predicated 128-bit load INTO the registers of v (no copy of the loaded value, so that the scoreboard
 // wait lands on the first real use, a stage later, and not on a loop-carried register move).
 __device__ __forceinline__ void ldg4_into(float4& v, const float* p, bool pred)
@@ -184,7 +180,7 @@ __device__ __forceinline__ void ldg4_into(float4& v, const float* p, bool pred)
         "{\n\t"
         ".reg .pred p;\n\t"
         "setp.ne.b32 p, %5, 0;\n\t"
-        "@p ld.global." FT_LDMODE ".v4.f32 {%0, %1, %2, %3}, [%4];\n\t"
+        "@p ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];\n\t"
         "}"
         : "+f"(v.x), "+f"(v.y), "+f"(v.z), "+f"(v.w)
         : "l"(p), "r"((int)pred));
@@ -194,9 +190,6 @@ __device__ __forceinline__ void stg4(float* p, float4 v) { *reinterpret_cast<flo
 // store the in-grid lanes of a quad starting at column x
 __device__ __forceinline__ void store_quad(float* p, float4 v, int x, int nx)
 {
-#ifdef EXP_NOSTORE
-    if (v.x != 123.456f) return;
-#endif
     if (x + 3 < nx) { stg4(p, v); return; }
     if (x < nx) p[0] = v.x;
     if (x + 1 < nx) p[1] = v.y;
@@ -230,12 +223,6 @@ __device__ __forceinline__ long long idx_z(const FusedArgs& a, int x, int y, int
 // memory (zeros outside the grid: a = 0 means no C-PML term ; b = 0 only ever multiplies zeros).
 // Helpers take pointers pre-offset so that t[i] is the value at grid index i (z: t[i & 15]).
 __device__ __forceinline__ float4 tab4(const float* t, int x) { return *reinterpret_cast<const float4*>(t + x); }
-__device__ __forceinline__ void prefetch_l2(const float* p)
-{
-#ifndef EXP_NOPF
-    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
-#endif
-}
 
 // Forward recursion on the thread's own quad (Eq. 46a / 46c with Eq. 38): m <- b m + a t ; returns t + m
 __device__ __forceinline__ float4 pml_fwd(const float* mi, float* mo, long long idx, float4 a4, float4 b4, float4 t, bool wr)
@@ -255,18 +242,12 @@ __device__ __forceinline__ float4 pml_fwd(const float* mi, float* mo, long long 
 __device__ __forceinline__ float4 pml_fwd_m(float4 m_old, float* mo, long long idx, float4 a4, float4 b4, float4 t, bool wr)
 {
     const float4 m = fma4(b4, m_old, a4 * t);
-#ifdef EXP_PMLNOMEM
-    wr = wr && m.x == 123.456f;
-#endif
     if (wr) stg4(mo + idx, m);
     return t + m;
 }
 __device__ __forceinline__ float4 pml_fwd_m(float4 m_old, float* mo, long long idx, float a1, float b1, float4 t, bool wr)
 {
     const float4 m = fma4(b1, m_old, a1 * t);
-#ifdef EXP_PMLNOMEM
-    wr = wr && m.x == 123.456f;
-#endif
     if (wr) stg4(mo + idx, m);
     return t + m;
 }
@@ -502,10 +483,7 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
 #pragma unroll
             for (int k = 0; k < 9; ++k) pm[k] = f4(0.0f);
             if (bx || by || (pml && (kk - 2 < a.P || kk + 2 >= a.nz - 1 - a.P))) {
-                bool ok = pok && (unsigned)kk < (unsigned)a.nz;
-#ifdef EXP_PMLNOMEM
-                ok = false;
-#endif
+                const bool ok = pok && (unsigned)kk < (unsigned)a.nz;
                 const int pzk = ok ? yzslab_row(kk, a.nz, a.P) : -1;
                 const bool ex = ok && colq >= 0, ey = ok && prow >= 0, ez = pzk >= 0;
                 const long long ix = ex ? idx_x(a, colq, y, kk) : 0, iy = ey ? idx_y(a, x, prow, kk) : 0, iz = ez ? idx_z(a, x, y, pzk) : 0;
@@ -537,28 +515,6 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
             const int pz = (pml && zin) ? yzslab_row(kk, a.nz, a.P) : -1;
             const bool bz = pml && (kk - 2 < a.P || kk + 2 >= a.nz - 1 - a.P);
             const bool pml1 = (bx || by || bz) && pok && zin;
-
-            if (pml && pok && (unsigned)(kk + 2) < (unsigned)a.nz) {
-                // pull the memory variables of plane kk + 2 into L2 (there is no L1 left beside 227 KB of shared memory)
-                const int zp = kk + 2;
-                const bool psi = MODE == FM_ADJ || inner;      // forward: psi is only touched by the owner
-                if (colq >= 0) {
-                    const long long i = idx_x(a, colq, y, zp);
-                    prefetch_l2(a.mvi[0] + i); prefetch_l2(a.mvi[3] + i); prefetch_l2(a.mvi[6] + i);
-                    if (psi) { prefetch_l2(a.mvi[9] + i); prefetch_l2(a.mvi[12] + i); prefetch_l2(a.mvi[15] + i); }
-                }
-                if (prow >= 0) {
-                    const long long i = idx_y(a, x, prow, zp);
-                    prefetch_l2(a.mvi[1] + i); prefetch_l2(a.mvi[4] + i); prefetch_l2(a.mvi[7] + i);
-                    if (psi) { prefetch_l2(a.mvi[10] + i); prefetch_l2(a.mvi[13] + i); prefetch_l2(a.mvi[16] + i); }
-                }
-                const int pzp = yzslab_row(zp, a.nz, a.P);
-                if (pzp >= 0) {
-                    const long long i = idx_z(a, x, y, pzp);
-                    prefetch_l2(a.mvi[2] + i); prefetch_l2(a.mvi[5] + i); prefetch_l2(a.mvi[8] + i);
-                    if (psi) { prefetch_l2(a.mvi[11] + i); prefetch_l2(a.mvi[14] + i); prefetch_l2(a.mvi[17] + i); }
-                }
-            }
 
             // staggered coefficients (reading G10): J = 1 - dt alpha_b, B = dt/(h rho_b)
             const float4 r0 = ld4s(PR, q), a0 = ld4s(PA, q);
@@ -667,10 +623,7 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
 #pragma unroll
             for (int k = 0; k < 9; ++k) qm[k] = f4(0.0f);
             if (bx || by || (pml && (kk - 4 < a.P || kk >= a.nz - 1 - a.P))) {
-                bool ok = inner && it >= 4;
-#ifdef EXP_PMLNOMEM
-                ok = false;
-#endif
+                const bool ok = inner && it >= 4;
                 const int pzk = ok ? yzslab_row(kk - 2, a.nz, a.P) : -1;
                 const bool ex = ok && colq >= 0, ey = ok && prow >= 0, ez = pzk >= 0;
                 const long long ix = ex ? idx_x(a, colq, y, kk - 2) : 0, iy = ey ? idx_y(a, x, prow, kk - 2) : 0, iz = ez ? idx_z(a, x, y, pzk) : 0;
@@ -686,9 +639,9 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
         __syncthreads();
         // every thread is past stage 1 of `it` and stage 2 of `it - 1`: refill the slots they freed
         if (tid == 0) {
-            if (it + 2 < itn) issueG(it + 2);
+            if (it + 1 < itn) issueU(it + 1);   // needed first ; slot of plane it - 4: its last cross-thread reads were in stage 2 of it - 2
             if (it + 2 <= itn) issueM(it);
-            if (it + 1 < itn) issueU(it + 1);   // slot of plane it - 4: its last cross-thread reads were in stage 2 of it - 2
+            if (it + 2 < itn) issueG(it + 2);
         }
         if (it >= 1) mbar_wait(&barM[(it - 1) % 3], ((it - 1) / 3) & 1);
         // ------------------------------------------------------------------ stage 2: sigma(ks), ks = kk - 2
@@ -701,7 +654,7 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
             const float* U1p = sm + FT_OFF_UR + 0 * FT_RING * FT_UPL;
             const float* U2p = sm + FT_OFF_UR + 1 * FT_RING * FT_UPL;
             const float* U3p = sm + FT_OFF_UR + 2 * FT_RING * FT_UPL;
-            const int p0 = (j % FT_RING) * FT_UPL, pm1 = ((j + 4) % FT_RING) * FT_UPL, pm2 = ((j + 3) % FT_RING) * FT_UPL;
+            const int p0 = (j % FT_RING) * FT_UPL, pm1 = ((j + 4) % FT_RING) * FT_UPL;
             const int pp1 = ((j + 1) % FT_RING) * FT_UPL, pp2 = ((j + 2) % FT_RING) * FT_UPL;
             const int pz = pml ? yzslab_row(ks, a.nz, a.P) : -1;
             const bool bz = pml && (ks - 2 < a.P || ks + 2 >= a.nz - 1 - a.P);

@@ -11,7 +11,7 @@
 
 // ---- pact_create: scan the caller's volumes -----------------------------------------------------
 // flags bit 0: non-finite value ; bit 1: rho <= 0 ; bit 2: mu < 0 ; bit 3: lambda + 2 mu <= 0 ;
-// bit 4: alpha < 0.  cmax2 = max (lambda + 2 mu)/rho as float bits (positive floats order as ints).
+// bit 4: alpha < 0 ; bit 5: 3 lambda + 2 mu <= 0 (legal, but the fused adjoint divides by it).  cmax2 = max (lambda + 2 mu)/rho as float bits (positive floats order as ints).
 __global__ void k_scan_materials(const float* __restrict__ lam, const float* __restrict__ mu,
                                  const float* __restrict__ rho, const float* __restrict__ alpha,
                                  long long N, unsigned int* flags, unsigned int* cmax2_bits)
@@ -26,6 +26,7 @@ __global__ void k_scan_materials(const float* __restrict__ lam, const float* __r
         if (m < 0.0f) f |= 4u;
         if (!(l + 2.0f * m > 0.0f)) f |= 8u;
         if (a < 0.0f) f |= 16u;
+        if (!(3.0f * l + 2.0f * m > 0.0f)) f |= 32u;   // not an error: only rules out the scaled adjoint variables of the fused path
         if (r > 0.0f) c2 = fmaxf(c2, (l + 2.0f * m) / r);
     }
     for (int o = 16; o > 0; o >>= 1) {

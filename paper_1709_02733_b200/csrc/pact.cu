@@ -21,7 +21,6 @@
 #include "kernels_plain.cuh"
 #include "kernels_fused.cuh"
 
-#define PACT_DEFAULT_VARIANT 1
 
 // ------------------------------------------------------------------------------------------------
 static thread_local char g_cuda_err[512] = "";
@@ -59,6 +58,7 @@ struct pact_ctx {
     long long state_bytes;
     float* scratch_base;     // adjoint scratch of the plain variant, allocated on first use
     // fused variant (kernels_fused.cuh): second state buffer, ping-pong memory variables, TMA maps
+    bool bulk_positive;      // 3 lambda + 2 mu > 0 everywhere (the fused adjoint carries C sigma_bar and divides by it)
     bool fused_ready;
     DevGrid g2;              // view of state buffer B for the I/O kernels
     float* stateB_base;
@@ -193,7 +193,8 @@ static int create_impl(pact_ctx* c, const pact_params* prm, const float* lam, co
     unsigned int h_scan[2];
     CK(cudaMemcpyAsync(h_scan, d_scan, sizeof(h_scan), cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
-    if (h_scan[0]) return PACT_EMATERIAL;
+    if (h_scan[0] & 31u) return PACT_EMATERIAL;
+    c->bulk_positive = !(h_scan[0] & 32u);
     float c2;
     memcpy(&c2, &h_scan[1], sizeof(float));
     const double cmax = std::sqrt((double)c2);
@@ -365,7 +366,16 @@ struct Launcher {
     }
 };
 
-static int resolve_variant(const pact_ctx* c) { return c->variant == 0 ? PACT_DEFAULT_VARIANT : c->variant; }
+// 1 = plain two-kernel path, 2 = fused single-pass path.  Automatic: the fused kernel runs one CTA per SM over
+// 32 x 32 x (>= 32) bricks, so it needs a grid with at least one brick per SM; smaller grids (which fit in L2 and
+// are launch/latency bound anyway) take the one-thread-per-cell kernels.
+static int resolve_variant(const pact_ctx* c)
+{
+    if (!c->bulk_positive) return 1;
+    if (c->variant != 0) return c->variant;
+    const long long bricks = (long long)((c->prm.nx + FT_TX - 1) / FT_TX) * ((c->prm.ny + FT_TY - 1) / FT_TY) * ((c->prm.nz + 31) / 32);
+    return bricks >= 148 ? 2 : 1;
+}
 
 static int ensure_scratch(pact_ctx* c)
 {

@@ -124,6 +124,30 @@ def test_fused_z_chunking(torch_cuda, zchunk):
     assert rel_l2(Hty, Hty_o) <= TOL_L2
 
 
+def test_automatic_variant_and_negative_lambda(torch_cuda):
+    """variant 0 picks the fused path on a grid with >= 148 bricks of 32^3 and the plain path below;
+    a medium with 3 lambda + 2 mu < 0 (legal: lambda + 2 mu > 0) must not take the scaled adjoint."""
+    from dataclasses import replace
+    prob = synth.random_problem(nx=192, ny=160, nz=170, nt=8, npml=6, L=11, seed=23, lossy=True)   # 6*5*6 = 180 bricks
+    x, y = synth.random_vectors(prob, seed=23)
+    ctx = gpu_ops(torch_cuda, prob, variant=0, graph=0)
+    ctx.set_option("profile", 1)
+    xd = torch_cuda.from_numpy(x.astype(np.float32)).cuda()
+    Hx = ctx.forward(xd).cpu().numpy()
+    _, km, _ = ctx.timing("forward")
+    assert km["fwd_fused"] > 0 and km["fwd_vel"] == 0
+    ctx.close()
+    Hx_o, _ = oracle_pair(prob, x, np.zeros_like(y))
+    assert rel_l2(Hx, Hx_o) <= TOL_L2
+    small = synth.random_problem(nx=40, ny=36, nz=33, nt=12, npml=4, L=5, seed=24, lossy=True)
+    mu = small.mu.copy(); mu[mu == 0] = mu.max() * 0.1
+    aux = replace(small, mu=mu, lam=(-0.8 * mu).astype(np.float32))   # lambda + 2 mu = 1.2 mu > 0 ; 3 lambda + 2 mu < 0
+    x, y = synth.random_vectors(aux, seed=24)
+    Hx, Hty = run_pair(torch_cuda, aux, x, y, variant=2)               # asks for fused, gets the plain path
+    Hx_o, Hty_o = oracle_pair(aux, x, y)
+    assert rel_l2(Hx, Hx_o) <= TOL_L2 and rel_l2(Hty, Hty_o) <= TOL_L2
+
+
 def test_graph_and_direct_launch_agree_bitwise(torch_cuda):
     prob = synth.random_problem(nx=40, ny=24, nz=33, nt=30, npml=4, L=7, seed=6)
     x, y = synth.random_vectors(prob, seed=6)
