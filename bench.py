@@ -60,7 +60,7 @@ def cpu_sample(prob):
     from paper_1709_02733_b200 import synth
     n_full = prob.prm.nx
     n = min(n_full, 160)
-    nt = 12 if n_full > n else min(prob.prm.nt, 12)
+    nt = 200 if n_full > n else min(prob.prm.nt, 200)      # ~15-20 s of oracle work at 0.1 Gcell-updates/s
     if n_full > n:
         # block under the top of the hemispherical array: contains water, porous skull and receivers
         x0 = y0 = (n_full - n) // 2
@@ -74,9 +74,9 @@ def cpu_sample(prob):
     return sub, what
 
 
-def time_oracle(sub, repeats=2):
+def time_oracle(sub, repeats=1):
     """Seconds for one forward + one adjoint of the oracle on `sub` (as it stands, OpenMP threads);
-    best of `repeats` (the first pass also pays page faults and thread start-up)."""
+    best of `repeats`."""
     import numpy as np
     from oracle.oracle import Oracle, threads
     o = Oracle.from_problem(sub)
@@ -169,6 +169,24 @@ class ClockSampler:
         return out
 
 
+def max_over_ranks(value, world, device=None):
+    """MAX of a per-rank scalar over all ranks (the slowest rank defines the time of a multi-GPU step).
+    Uses the default process group (NCCL on GPUs; gloo in the CPU tests); identity for world = 1."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(cells_per_rank_step, steps, world, ms_max):
+    """Replicas only: every rank processes its own copy of the workload, so the job's cell updates are
+    world x (one rank's), divided by the slowest rank's device time.  Gcell-updates/s."""
+    return world * cells_per_rank_step * steps / (ms_max * 1e-3) / 1e9
+
+
 def peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -233,12 +251,9 @@ def main():
     torch.cuda.synchronize(dev)
     barrier()
     clk = clocks.stop() if rank == 0 else None
-    ms = torch.tensor([ev0.elapsed_time(ev1)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
-    ms = float(ms.item())
+    ms = max_over_ranks(ev0.elapsed_time(ev1), world, dev)
     cells_step = 2.0 * prm.N * (prm.nt - 1)                # forward + adjoint
-    value = world * cells_step * args.steps / (ms * 1e-3) / 1e9
+    value = whole_job_rate(cells_step, args.steps, world, ms)
 
     # ---- roofline of the step kernels, from the library's own CUDA events in the timed region
     loop_f, k_f, n_f = ctx.timing("forward")
@@ -264,7 +279,11 @@ def main():
         tr = os.path.join(ROOT, "profiles", "traffic.json")   # per-launch DRAM bytes from the committed ncu capture
         if os.path.exists(tr):
             try:
-                roof["traffic"] = json.load(open(tr)).get(f"config{args.config}")
+                t = json.load(open(tr)).get(f"config{args.config}")
+                # per launch of the dominant kernel (the adjoint step), from the committed ncu --set full capture
+                roof["traffic"] = t["adjoint_bytes_per_launch"] / 1e9 if t else None
+                roof["traffic_unit"] = "GB per launch (dram__bytes_read.sum + dram__bytes_write.sum), algorithmic %.2f" % (B_ALG * prm.N / 1e9)
+                roof["traffic_forward"] = t["forward_bytes_per_launch"] / 1e9 if t else None
             except Exception:
                 pass
 
@@ -282,11 +301,9 @@ def main():
             ctx.forward_host(p0_h, data_h)
             ctx.adjoint_host(data_h, image_h)
         torch.cuda.synchronize(dev)
-        t_e = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(t_e, op=dist.ReduceOp.MAX)
+        t_e = max_over_ranks(time.perf_counter() - t0, world, dev)
         nb = prm.N * 4 + prm.nt * prob.L * 4
-        e2e = {"value": world * cells_step * n_e2e / float(t_e.item()) / 1e9, "unit": UNIT,
+        e2e = {"value": whole_job_rate(cells_step, n_e2e, world, t_e * 1e3), "unit": UNIT,
                "h2d_bytes_per_step": nb, "d2h_bytes_per_step": nb, "steps": n_e2e,
                "api": "pact_forward_host + pact_adjoint_host (pinned host buffers)"}
 

@@ -148,6 +148,32 @@ def test_automatic_variant_and_negative_lambda(torch_cuda):
     assert rel_l2(Hx, Hx_o) <= TOL_L2 and rel_l2(Hty, Hty_o) <= TOL_L2
 
 
+@pytest.mark.slow
+def test_config4_full_size_truncated(torch_cuda):
+    """BASELINE config 4 at its full 512^3 size on its real volumes (porous skull, 16-cell C-PML, 4096
+    hemispherical receivers), in the launch configuration bench.py times (automatic variant = fused, no graph),
+    truncated to 8 samples so that the oracle finishes in about a minute.  Random x over the whole grid and
+    random y, so the C-PML slabs and every receiver carry signal."""
+    prob = synth.make_config(4, nt=8)
+    x, y = synth.random_vectors(prob, seed=44)
+    ctx = gpu_ops(torch_cuda, prob, variant=0)
+    ctx.set_option("profile", 1)
+    xd = torch_cuda.from_numpy(np.ascontiguousarray(x, dtype=np.float32)).cuda()
+    yd = torch_cuda.from_numpy(np.ascontiguousarray(y, dtype=np.float32)).cuda()
+    Hx = ctx.forward(xd).cpu().numpy()
+    Hty = ctx.adjoint(yd).cpu().numpy()
+    _, km, _ = ctx.timing("adjoint")
+    assert km["adj_fused"] > 0                       # the fused kernel is what ran
+    ctx.close()
+    del xd, yd
+    Hx_o, Hty_o = oracle_pair(prob, x, y)
+    assert rel_l2(Hx, Hx_o) <= TOL_L2
+    assert rel_l2(Hty, Hty_o) <= TOL_L2
+    x32, y32 = x.astype(np.float32).astype(np.float64), y.astype(np.float32).astype(np.float64)
+    a, b = np.vdot(Hx.astype(np.float64), y32), np.vdot(x32, Hty.astype(np.float64))
+    assert abs(a - b) <= TOL_DOT * max(abs(a), abs(b))
+
+
 def test_graph_and_direct_launch_agree_bitwise(torch_cuda):
     prob = synth.random_problem(nx=40, ny=24, nz=33, nt=30, npml=4, L=7, seed=6)
     x, y = synth.random_vectors(prob, seed=6)
