@@ -69,9 +69,7 @@
 
 struct FusedArgs {
     int nx, ny, nz;
-    int ntx, nty;          // tiles along x, y
-    int zc;                // planes per z chunk
-    int nzc;               // chunks
+    const int4* work;      // CTA b processes tile (work[b].x, work[b].y), planes [work[b].z, work[b].w)
     long long sy, sz, box; // strides (elements) of the padded box; elements per field
     const float* in;       // state read  (field k at in + k*box; pointer to node (0,0,0))
     float* out;            // state written
@@ -345,11 +343,9 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
     uint64_t* barU = bars + 5;    // [2]  u_old of plane c, landed in ring slot c % FT_RING -> barrier c & 1
 
     const int tid = threadIdx.x;
-    int b = blockIdx.x;
-    const int tx = b % a.ntx; b /= a.ntx;
-    const int ty = b % a.nty; b /= a.nty;
-    const int zb = b * a.zc, ze = min(zb + a.zc, a.nz);
-    const int x0 = tx * FT_TX, y0 = ty * FT_TY;
+    const int4 wk = __ldg(a.work + blockIdx.x);
+    const int zb = wk.z, ze = wk.w;
+    const int x0 = wk.x * FT_TX, y0 = wk.y * FT_TY;
     const int itn = ze - zb + 4;            // iterations: u planes kk = zb-2 .. ze+1
 
     // thread -> quad of the u region (10 quads x 36 rows)

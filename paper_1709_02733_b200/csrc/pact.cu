@@ -66,6 +66,14 @@ struct pact_ctx {
     CUtensorMap tmS40[2], tmS36[2], tmM40, tmM36;
     FusedArgs fa;
     int zchunk;              // planes per CTA along z (0 = auto)
+    // work lists of the fused launches: [0] CTAs whose bricks (with every tap of the adjoint) stay clear of the
+    // C-PML slabs (run without any C-PML code), [1] all the others
+    int4* d_work[2];
+    int nwork[2];
+    int work_zc;             // zchunk value the lists were built for (-1 = not built)
+    long long work_cap;
+    cudaStream_t aux_stream; // the slab CTAs run beside the interior ones
+    cudaEvent_t ev_fork, ev_join;
     float* mvbuf[2][18];     // fused memory variables, two sets (read / written alternate every step)
     // host-buffer variants
     float* d_vol;            // [N]
@@ -139,6 +147,9 @@ extern "C" void pact_destroy(pact_ctx* c)
     cudaStreamSynchronize(c->stream);
     free_graphs(c);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
+    if (c->aux_stream) cudaStreamDestroy(c->aux_stream);
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    if (c->ev_join) cudaEventDestroy(c->ev_join);
     for (int op = 0; op < 2; ++op) {
         for (int k = 0; k < 8; ++k)
             for (auto& s : c->samples[op][k]) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
@@ -440,7 +451,6 @@ static int ensure_fused(pact_ctx* c)
     FusedArgs& fa = c->fa;
     memset(&fa, 0, sizeof(fa));
     fa.nx = g.nx; fa.ny = g.ny; fa.nz = g.nz;
-    fa.ntx = (g.nx + FT_TX - 1) / FT_TX; fa.nty = (g.ny + FT_TY - 1) / FT_TY;
     fa.sy = g.sy; fa.sz = g.sz; fa.box = c->box;
     fa.P = P;
     fa.nxq = (g.nx + 3) / 4 * 4;
@@ -495,7 +505,69 @@ static int ensure_fused(pact_ctx* c)
     CK(cudaFuncSetAttribute(k_fused<FM_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
     CK(cudaFuncSetAttribute(k_fused<FM_ADJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
     fa.mat = g.Ll;
+    c->work_zc = -1;
+    c->work_cap = (long long)((g.nx + FT_TX - 1) / FT_TX) * ((g.ny + FT_TY - 1) / FT_TY) * (g.nz + 2);
+    for (int k = 0; k < 2; ++k)
+        if ((rc = dev_alloc(c, (void**)&c->d_work[k], (size_t)c->work_cap * sizeof(int4)))) return rc;
+    CK(cudaStreamCreateWithFlags(&c->aux_stream, cudaStreamNonBlocking));
+    CK(cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
+    CK(cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
     c->fused_ready = true;
+    return PACT_OK;
+}
+
+// z chunks of [z0, z1) for `tiles` tiles: `zc` planes each, or (zc <= 0) the chunk count that minimises
+// waves x (planes per chunk + 4 start-up planes) for one CTA per SM, chunks no shorter than 32 planes
+static int chunk_len(int z0, int z1, long long tiles, int zc)
+{
+    const int n = z1 - z0;
+    if (n <= 0) return 1;
+    if (zc > 0) return std::min(zc, n);
+    long long best = -1;
+    int len = n;
+    for (int k = 1; k <= std::max(1, n / 32); ++k) {
+        const int z = (n + k - 1) / k;
+        const long long ctas = tiles * ((n + z - 1) / z);
+        const long long cost = ((ctas + 147) / 148) * (z + 4);
+        if (best < 0 || cost < best) { best = cost; len = z; }
+    }
+    return len;
+}
+
+// Work lists: a brick is "interior" when its u region with the +-2 taps of the
+// transposed C-PML recursion (x0-4 .. x0+35, likewise y, planes zb-4 .. ze+2) misses every slab; such bricks
+// run the kernel without C-PML code.  Everything else (boundary tiles over all z; the z slabs of interior
+// tiles) runs the C-PML kernel on a second stream beside it.
+static int build_work(pact_ctx* c)
+{
+    if (c->work_zc == c->zchunk) return PACT_OK;
+    const DevGrid& g = c->g;
+    const int P = g.P, ntx = (g.nx + FT_TX - 1) / FT_TX, nty = (g.ny + FT_TY - 1) / FT_TY;
+    std::vector<int4> wl[2];
+    auto interior_1d = [&](int t0, int n) { return P == 0 || (t0 - 4 >= P && t0 + 36 <= n - 1 - P); };
+    int zlo = 0, zhi = g.nz;
+    if (P > 0) { zlo = P + 4; zhi = g.nz - 5 - P; }
+    std::vector<std::pair<int, int>> tin, tbd;
+    for (int ty = 0; ty < nty; ++ty)
+        for (int tx = 0; tx < ntx; ++tx)
+            ((interior_1d(tx * FT_TX, g.nx) && interior_1d(ty * FT_TY, g.ny) && zhi - zlo >= 8) ? tin : tbd).push_back({tx, ty});
+    auto add = [&](std::vector<int4>& w, const std::vector<std::pair<int, int>>& tiles, int z0, int z1) {
+        if (tiles.empty() || z1 <= z0) return;
+        const int len = chunk_len(z0, z1, (long long)tiles.size(), c->zchunk);
+        for (int zb = z0; zb < z1; zb += len)               // chunk-major: neighbouring tiles march the same planes together
+            for (auto& t : tiles) w.push_back(make_int4(t.first, t.second, zb, std::min(zb + len, z1)));
+    };
+    add(wl[0], tin, zlo, zhi);
+    add(wl[1], tbd, 0, g.nz);
+    if (P > 0) { add(wl[1], tin, 0, zlo); add(wl[1], tin, zhi, g.nz); }
+    for (int k = 0; k < 2; ++k) {
+        if ((long long)wl[k].size() > c->work_cap) return PACT_EINVAL;
+        c->nwork[k] = (int)wl[k].size();
+        if (!wl[k].empty())
+            CK(cudaMemcpyAsync(c->d_work[k], wl[k].data(), wl[k].size() * sizeof(int4), cudaMemcpyHostToDevice, c->stream));
+    }
+    CK(cudaStreamSynchronize(c->stream));   // the vectors are temporaries
+    c->work_zc = c->zchunk;
     return PACT_OK;
 }
 
@@ -508,29 +580,31 @@ static void fused_step(pact_ctx* c, Launcher& ln, int cur, float sgn, int kind)
     fa.in = gi.f[0]; fa.out = go.f[0];
     fa.sgn = sgn;
     for (int k = 0; k < 18; ++k) { fa.mvi[k] = c->mvbuf[cur][k]; fa.mvo[k] = c->mvbuf[1 - cur][k]; }
-    int zc = c->zchunk;
-    if (zc <= 0) {
-        // z chunks: one CTA per SM and 4 start-up planes per chunk; take the chunk count that minimises
-        // waves x (planes per chunk + 4), chunks no shorter than 32 planes
-        const int tiles = fa.ntx * fa.nty;
-        long long best = -1;
-        for (int nzc = 1; nzc <= std::max(1, fa.nz / 32); ++nzc) {
-            const int z = (fa.nz + nzc - 1) / nzc;
-            const long long ctas = (long long)tiles * ((fa.nz + z - 1) / z);
-            const long long cost = ((ctas + 147) / 148) * (z + 4);
-            if (best < 0 || cost < best) { best = cost; zc = z; }
-        }
+    cudaStream_t st = c->stream, aux = c->aux_stream;
+    const bool both = c->nwork[0] > 0 && c->nwork[1] > 0;
+    if (both) { cudaEventRecord(c->ev_fork, st); cudaStreamWaitEvent(aux, c->ev_fork, 0); }
+    if (c->nwork[1] > 0) {      // the slab CTAs (slower per plane) start first
+        FusedArgs fb = fa;
+        fb.work = c->d_work[1];
+        cudaStream_t s1 = both ? aux : st;
+        const int grid = c->nwork[1];
+        auto launch = [&] {
+            if (fa.P == 0) k_fused<FM_PLAIN><<<grid, FT_NT, FT_SMEM_BYTES, s1>>>(c->tmS40[cur], c->tmS36[cur], c->tmM40, c->tmM36, fb);
+            else if (sgn > 0.0f) k_fused<FM_FWD><<<grid, FT_NT, FT_SMEM_BYTES, s1>>>(c->tmS40[cur], c->tmS36[cur], c->tmM40, c->tmM36, fb);
+            else k_fused<FM_ADJ><<<grid, FT_NT, FT_SMEM_BYTES, s1>>>(c->tmS40[cur], c->tmS36[cur], c->tmM40, c->tmM36, fb);
+        };
+        if (both) { launch(); cudaEventRecord(c->ev_join, aux); }   // timed with the interior launch below (they overlap)
+        else ln.run(kind, launch);
     }
-    zc = std::max(1, std::min(zc, fa.nz));
-    fa.zc = zc; fa.nzc = (fa.nz + zc - 1) / zc;
-    const int grid = fa.ntx * fa.nty * fa.nzc;
-    cudaStream_t st = c->stream;
-    if (fa.P == 0)
-        ln.run(kind, [&] { k_fused<FM_PLAIN><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM40, c->tmM36, fa); });
-    else if (sgn > 0.0f)
-        ln.run(kind, [&] { k_fused<FM_FWD><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM40, c->tmM36, fa); });
-    else
-        ln.run(kind, [&] { k_fused<FM_ADJ><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM40, c->tmM36, fa); });
+    if (c->nwork[0] > 0) {
+        FusedArgs fb = fa;
+        fb.work = c->d_work[0];
+        const int grid = c->nwork[0];
+        ln.run(kind, [&] {
+            k_fused<FM_PLAIN><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM40, c->tmM36, fb);
+            if (both) cudaStreamWaitEvent(st, c->ev_join, 0);
+        });
+    }
 }
 
 // Eq. 58 right to left: tau, then for m = 0..M-1 { Theta ; W' unless m = M-1 }
@@ -603,6 +677,7 @@ static int run_loop(pact_ctx* c, int which /*0 fwd, 1 adj*/)
     if (variant == 2) {
         int rc = ensure_fused(c);
         if (rc) return rc;
+        if ((rc = build_work(c))) return rc;
         CK(cudaMemsetAsync(c->stateB_base, 0, (size_t)c->stateB_bytes, c->stream));
     }
     for (int k = 0; k < 8; ++k) { c->used[which][k] = 0; c->launches[which][k] = 0; }
