@@ -9,11 +9,12 @@
 // over a chunk of planes.  A thread owns one float4 (4 consecutive x) of one row.
 //   stage 1 (Eq. 46a,b): u(kk) on the tile + 2 cells of ring, from sigma on the tile + 4 cells;
 //   stage 2 (Eq. 46c,d): sigma(kk-2) on the tile, from u(kk-4 .. kk) kept in a shared-memory ring.
-// Fields whose x/y neighbours are needed (s11,s22,s12,s13,s23, rho, alpha, mu) and s33 arrive in
-// shared memory by TMA (cp.async.bulk.tensor, mbarrier complete_tx), two planes ahead of use; u_old(kk)
-// lands by TMA in the very ring slot that u_new(kk) then overwrites in place; the z neighbours of
-// s13,s23,s33 (and the oldest u3 tap) live in per-thread registers; lambda and the old s11,s22,s12
-// of stage 2 are own-column 128-bit loads issued one stage ahead of use (L2 hits but for lambda).
+// Fields whose x/y neighbours are needed (s11,s22,s12,s13,s23, rho, alpha, mu), s33 and lambda arrive in
+// shared memory by TMA (cp.async.bulk.tensor, mbarrier complete_tx), one or two planes ahead of use;
+// u_old(kk) lands by TMA in the very ring slot that u_new(kk) then overwrites in place; the z neighbours
+// of s13,s23,s33 (and the oldest u3 tap) live in per-thread registers; the old s11,s22,s12 of stage 2 are
+// own-column 128-bit loads issued one stage ahead of use (L2 hits: TMA fetched those planes two
+// iterations earlier).  Global loads through the LSU that miss L2 are what this kernel cannot afford.
 // The ring of 2 (4) cells around the tile is recomputed by the neighbouring CTAs; nothing is
 // exchanged between CTAs, hence the two state buffers.
 //
@@ -41,19 +42,24 @@
 #define FT_MW 36                      // mu box: tile + 1 (rounded up to a quad) in x
 #define FT_MH 33                      //         tile + 1 in y
 #define FT_MPL 1216                   // floats per mu plane buffer (36*33 = 1188, padded to 128 B)
+#define FT_RH 37                      // rows of the rho / alpha planes: u region + 1
+#define FT_RPL 1504                   // floats per rho / alpha plane buffer (40*37 = 1480, padded to 128 B)
+#define FT_LPL (FT_TX * FT_TY)        // floats per lambda plane (the tile itself)
 #define FT_RING 5                     // u planes in the ring: ks-1 .. ks+2 and the slot u_old(kk+1) is landing in
 
-// shared memory map (floats)
-#define FT_OFF_S11 0
-#define FT_OFF_S22 (FT_OFF_S11 + 2 * FT_BOX)
+// shared memory map (floats).  Planes are only as tall as their readers need: s11, s13 (x neighbours only) and
+// s33 (own column) cover the u region (36 rows), rho / alpha one row more, s22, s12, s23 the full 40.
+#define FT_OFF_S22 0
 #define FT_OFF_S12 (FT_OFF_S22 + 2 * FT_BOX)
-#define FT_OFF_S13 (FT_OFF_S12 + 2 * FT_BOX)
-#define FT_OFF_S23 (FT_OFF_S13 + 3 * FT_BOX)
+#define FT_OFF_S11 (FT_OFF_S12 + 2 * FT_BOX)
+#define FT_OFF_S13 (FT_OFF_S11 + 2 * FT_UPL)
+#define FT_OFF_S23 (FT_OFF_S13 + 3 * FT_UPL)
 #define FT_OFF_RHO (FT_OFF_S23 + 3 * FT_BOX)
-#define FT_OFF_ALP (FT_OFF_RHO + 3 * FT_BOX)
-#define FT_OFF_S33 (FT_OFF_ALP + 3 * FT_BOX)
+#define FT_OFF_ALP (FT_OFF_RHO + 3 * FT_RPL)
+#define FT_OFF_S33 (FT_OFF_ALP + 3 * FT_RPL)
 #define FT_OFF_MU (FT_OFF_S33 + 2 * FT_UPL)
-#define FT_OFF_UR (FT_OFF_MU + 3 * FT_MPL)
+#define FT_OFF_LAM (FT_OFF_MU + 3 * FT_MPL)
+#define FT_OFF_UR (FT_OFF_LAM + 2 * FT_LPL)
 #define FT_OFF_END (FT_OFF_UR + 3 * FT_RING * FT_UPL)
 #define FT_TABW 48                     // x / y C-PML table window: tile - 8 .. tile + 39
 #define FT_ZRING 16                   // z C-PML table ring (planes)
@@ -334,7 +340,8 @@ __device__ __forceinline__ void adj_own(const float* Ti, float* To, long long i,
 template <int MODE>
 __global__ void __launch_bounds__(FT_NT, 1)
 k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUtensorMap tmS36,
-        const __grid_constant__ CUtensorMap tmM40, const __grid_constant__ CUtensorMap tmM36, const FusedArgs a)
+        const __grid_constant__ CUtensorMap tmM37, const __grid_constant__ CUtensorMap tmM36,
+        const __grid_constant__ CUtensorMap tmL, const FusedArgs a)
 {
     extern __shared__ __align__(1024) float sm[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(sm + FT_OFF_END);
@@ -402,17 +409,18 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
     // E(j): s13, s23, rho, alpha of plane j -> slot j % 3
     auto issueE = [&](int j, uint64_t* bar) {
         const int s = j % 3;
-        tma_plane(&tmS40, sm + FT_OFF_S13 + s * FT_BOX, bar, cx40, cy40, cz0 + j, S13);
+        tma_plane(&tmS36, sm + FT_OFF_S13 + s * FT_UPL, bar, cx40, cy36, cz0 + j, S13);
         tma_plane(&tmS40, sm + FT_OFF_S23 + s * FT_BOX, bar, cx40, cy40, cz0 + j, S23);
-        tma_plane(&tmM40, sm + FT_OFF_RHO + s * FT_BOX, bar, cx40, cy40, cz0 + j, 2);
-        tma_plane(&tmM40, sm + FT_OFF_ALP + s * FT_BOX, bar, cx40, cy40, cz0 + j, 3);
+        tma_plane(&tmM37, sm + FT_OFF_RHO + s * FT_RPL, bar, cx40, cy36, cz0 + j, 2);
+        tma_plane(&tmM37, sm + FT_OFF_ALP + s * FT_RPL, bar, cx40, cy36, cz0 + j, 3);
     };
     // group c = what stage 1 of iteration c reads for the first time:
     //   s11, s22, s12 of plane c -> slot c & 1 ; E(c + 1) ; s33 of plane c + 2 -> slot c & 1 ; (c = 0: E(0) too)
     auto issueG = [&](int c) {
         uint64_t* bar = &barG[c & 1];
-        mbar_expect_tx(bar, (7 * FT_BOX + FT_UPL + (c == 0 ? 4 * FT_BOX : 0)) * 4);
-        tma_plane(&tmS40, sm + FT_OFF_S11 + (c & 1) * FT_BOX, bar, cx40, cy40, cz0 + c, S11);
+        const uint32_t eBytes = (FT_UPL + FT_BOX + 2 * FT_BW * FT_RH) * 4;     // s13, s23, rho, alpha
+        mbar_expect_tx(bar, (2 * FT_UPL + 2 * FT_BOX) * 4 + eBytes + (c == 0 ? eBytes : 0));
+        tma_plane(&tmS36, sm + FT_OFF_S11 + (c & 1) * FT_UPL, bar, cx40, cy36, cz0 + c, S11);
         tma_plane(&tmS40, sm + FT_OFF_S22 + (c & 1) * FT_BOX, bar, cx40, cy40, cz0 + c, S22);
         tma_plane(&tmS40, sm + FT_OFF_S12 + (c & 1) * FT_BOX, bar, cx40, cy40, cz0 + c, S12);
         issueE(c + 1, bar);
@@ -421,8 +429,10 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
     };
     auto issueM = [&](int j) {
         uint64_t* bar = &barM[j % 3];
-        mbar_expect_tx(bar, FT_MW * FT_MH * 4);
+        mbar_expect_tx(bar, (FT_MW * FT_MH + FT_LPL) * 4);
         tma_plane(&tmM36, sm + FT_OFF_MU + (j % 3) * FT_MPL, bar, cxm, cym, cz0 + j, 1);
+        // lambda of plane j - 1 (read by stage 2 of iteration j + 1, which waits on this barrier) -> slot (j - 1) & 1
+        tma_plane(&tmL, sm + FT_OFF_LAM + ((j + 1) & 1) * FT_LPL, bar, cxm, cym, cz0 + j - 1, 0);
     };
 
     // u_old(c) lands in the ring slot that u_new(c) will overwrite in place (own quads only)
@@ -441,7 +451,7 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
     float4 w23a, w23b, w23c;          // s23
     float4 w33a, w33b, w33c, w33d;    // s33 at kk-2, kk-1, kk, kk+1
     float4 u3m2 = f4(0.0f);           // u3(ks-2) of the thread's quad (its ring slot is refilled with u_old by then)
-    float4 lam, so11, so22, so12;     // lambda, old s11, s22, s12 at ks = kk - 2
+    float4 so11, so22, so12;          // old s11, s22, s12 at ks = kk - 2
     const float4 z4 = f4(0.0f);
     {
         const long long g = (long long)(zb - 2) * a.sz + gxy;
@@ -455,7 +465,7 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
         w33b = ld_ok ? ldg4(in + S33 * box + g - a.sz) : z4;
         w33c = ld_ok ? ldg4(in + S33 * box + g) : z4;
         w33d = ld_ok ? ldg4(in + S33 * box + g + a.sz) : z4;
-        lam = so11 = so22 = so12 = z4;
+        so11 = so22 = so12 = z4;
     }
 
     // coefficient scales: sign of the step and the 1/c2 of the unnormalised differences (d1)
@@ -495,14 +505,14 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
         const bool zin = (unsigned)kk < (unsigned)a.nz;
         // ------------------------------------------------------------------ stage 1: u(kk)
         if (act1) {
-            const float* P11 = sm + FT_OFF_S11 + (it & 1) * FT_BOX;
+            const float* P11 = sm + FT_OFF_S11 + (it & 1) * FT_UPL;
             const float* P22 = sm + FT_OFF_S22 + (it & 1) * FT_BOX;
             const float* P12 = sm + FT_OFF_S12 + (it & 1) * FT_BOX;
-            const float* P13 = sm + FT_OFF_S13 + s3 * FT_BOX;
+            const float* P13 = sm + FT_OFF_S13 + s3 * FT_UPL;
             const float* P23 = sm + FT_OFF_S23 + s3 * FT_BOX;
-            const float* PR = Rbase + s3 * FT_BOX;
-            const float* PA = Abase + s3 * FT_BOX;
-            f13 = ld4s(sm + FT_OFF_S13 + s3n * FT_BOX, q);
+            const float* PR = Rbase + s3 * FT_RPL;
+            const float* PA = Abase + s3 * FT_RPL;
+            f13 = ld4s(sm + FT_OFF_S13 + s3n * FT_UPL, uq);
             f23 = ld4s(sm + FT_OFF_S23 + s3n * FT_BOX, q);
             f33 = ld4s(sm + FT_OFF_S33 + (it & 1) * FT_UPL, uq);   // plane kk+2
 
@@ -513,7 +523,7 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
             const bool pml1 = (bx || by || bz) && pok && zin;
 
             // staggered coefficients (reading G10): J = 1 - dt alpha_b, B = dt/(h rho_b)
-            const float4 r0 = ld4s(PR, q), a0 = ld4s(PA, q);
+            const float4 r0 = ld4s(PR, uq), a0 = ld4s(PA, uq);
             const float4 one = f4(1.0f), mh = f4(-0.5f);
             const float4 c12 = ld4s(P12, q);
             float4 n1, n2, n3;
@@ -522,8 +532,8 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
             float* const R2 = sm + FT_OFF_UR + (1 * FT_RING + sl) * FT_UPL + 4 * uq;
             float* const R3 = sm + FT_OFF_UR + (2 * FT_RING + sl) * FT_UPL + 4 * uq;
             {   // ---- u1 at (x+1/2, y, z): D+x s11, D-y s12, D-z s13
-                const float4 c11 = ld4s(P11, q);
-                const float2 l = ld2s(P11, 4 * q - 2), rr = ld2s(P11, 4 * q + 4);
+                const float4 c11 = ld4s(P11, uq);
+                const float2 l = ld2s(P11, 4 * uq - 2), rr = ld2s(P11, 4 * uq + 4);
                 const float4 ya = ld4s(P12, q - 20), yb = ld4s(P12, q - 10), yd = ld4s(P12, q + 10);
                 float4 t1 = dpx(l, c11, rr), t2 = d4(ya, yb, c12, yd), t3 = d4(w13a, w13b, w13c, f13);
                 if (MODE == FM_FWD && pml1) {
@@ -536,7 +546,7 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                     if (by) t2 = t2 + adj_y(a, a.mvi[10], a.mvo[10], YT(T_A_HALF), YT(T_B_HALF), x, y - 2, kk, 2, ya, yb, c12, yd, wr1);
                     if (bz) t3 = t3 + adj_z(a, a.mvi[11], a.mvo[11], ZT(T_A_HALF), ZT(T_B_HALF), x, y, kk - 2, 2, w13a, w13b, w13c, f13, wr1);
                 }
-                const float4 rxp = shl1(r0, PR[4 * q + 4]), axp = shl1(a0, PA[4 * q + 4]);
+                const float4 rxp = shl1(r0, PR[4 * uq + 4]), axp = shl1(a0, PA[4 * uq + 4]);
                 mbar_wait(&barU[it & 1], (it >> 1) & 1);      // u_old(kk) has landed in the ring slot
                 n1 = fma4(fma4(mh, a0 + axp, one), *reinterpret_cast<const float4*>(R1), (kB * rcp4(r0 + rxp)) * (t1 + t2 + t3));
             }
@@ -554,11 +564,11 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                     if (by) t2 = t2 + adj_y(a, a.mvi[13], a.mvo[13], YT(T_A_INT), YT(T_B_INT), x, y - 1, kk, 1, yb, c22, yc, yd, wr1);
                     if (bz) t3 = t3 + adj_z(a, a.mvi[14], a.mvo[14], ZT(T_A_HALF), ZT(T_B_HALF), x, y, kk - 2, 2, w23a, w23b, w23c, f23, wr1);
                 }
-                const float4 ryp = ld4s(PR, q + 10), ayp = ld4s(PA, q + 10);
+                const float4 ryp = ld4s(PR, uq + 10), ayp = ld4s(PA, uq + 10);
                 n2 = fma4(fma4(mh, a0 + ayp, one), *reinterpret_cast<const float4*>(R2), (kB * rcp4(r0 + ryp)) * (t1 + t2 + t3));
             }
             {   // ---- u3 at (x, y, z+1/2): D-x s13, D-y s23, D+z s33
-                const float2 l = ld2s(P13, 4 * q - 2), rr = ld2s(P13, 4 * q + 4);
+                const float2 l = ld2s(P13, 4 * uq - 2), rr = ld2s(P13, 4 * uq + 4);
                 const float4 ya = ld4s(P23, q - 20), yb = ld4s(P23, q - 10), yd = ld4s(P23, q + 10);
                 float4 t1 = dmx(l, w13c, rr), t2 = d4(ya, yb, w23c, yd), t3 = d4(w33b, w33c, w33d, f33);
                 if (MODE == FM_FWD && pml1) {
@@ -571,7 +581,7 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                     if (by) t2 = t2 + adj_y(a, a.mvi[16], a.mvo[16], YT(T_A_HALF), YT(T_B_HALF), x, y - 2, kk, 2, ya, yb, w23c, yd, wr1);
                     if (bz) t3 = t3 + adj_z(a, a.mvi[17], a.mvo[17], ZT(T_A_INT), ZT(T_B_INT), x, y, kk - 1, 1, w33b, w33c, w33d, f33, wr1);
                 }
-                const float4 rzp = ld4s(Rbase + s3n * FT_BOX, q), azp = ld4s(Abase + s3n * FT_BOX, q);
+                const float4 rzp = ld4s(Rbase + s3n * FT_RPL, uq), azp = ld4s(Abase + s3n * FT_RPL, uq);
                 n3 = fma4(fma4(mh, a0 + azp, one), *reinterpret_cast<const float4*>(R3), (kB * rcp4(r0 + rzp)) * (t1 + t2 + t3));
             }
             if (edge_xy || !zin) {
@@ -717,6 +727,7 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
             const float4 mxy = kM * rcp4((i0 + ix) + (iy + ixy));
             const float4 mxz = kM * rcp4((i0 + ix) + (iz + ixz));
             const float4 myz = kM * rcp4((i0 + iy) + (iz + iyz));
+            const float4 lam = ld4s(sm + FT_OFF_LAM + (it & 1) * FT_LPL, (r - 2) * 8 + (qx - 1));   // lambda(ks), by TMA
             const float4 ldiv = (kL * lam) * (e11 + e22 + e33);
             const float4 n11 = so11 + fma4(mn2, e11, ldiv);
             const float4 n22 = so22 + fma4(mn2, e22, ldiv);
@@ -735,7 +746,6 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
         {   // own-column inputs of the next stage 2 (plane ks + 1)
             const bool p = inner && it >= 3 && it + 1 < itn;
             const long long g = (long long)(ks + 1) * a.sz + gxy;
-            ldg4_into(lam, a.mat + g, p);
             ldg4_into(so11, in + S11 * box + g, p);
             ldg4_into(so22, in + S22 * box + g, p);
             ldg4_into(so12, in + S12 * box + g, p);

@@ -63,7 +63,7 @@ struct pact_ctx {
     DevGrid g2;              // view of state buffer B for the I/O kernels
     float* stateB_base;
     long long stateB_bytes;
-    CUtensorMap tmS40[2], tmS36[2], tmM40, tmM36;
+    CUtensorMap tmS40[2], tmS36[2], tmM37, tmM36, tmL;
     FusedArgs fa;
     int zchunk;              // planes per CTA along z (0 = auto)
     // work lists of the fused launches: [0] CTAs whose bricks (with every tap of the adjoint) stay clear of the
@@ -499,7 +499,8 @@ static int ensure_fused(pact_ctx* c)
     if ((rc = make_map(c, enc, &c->tmS36[0], baseA, NFIELD, FT_BW, FT_UH))) return rc;
     if ((rc = make_map(c, enc, &c->tmS40[1], baseB, NFIELD, FT_BW, FT_BH))) return rc;
     if ((rc = make_map(c, enc, &c->tmS36[1], baseB, NFIELD, FT_BW, FT_UH))) return rc;
-    if ((rc = make_map(c, enc, &c->tmM40, baseM, 4, FT_BW, FT_BH))) return rc;
+    if ((rc = make_map(c, enc, &c->tmM37, baseM, 4, FT_BW, FT_RH))) return rc;
+    if ((rc = make_map(c, enc, &c->tmL, baseM, 4, FT_TX, FT_TY))) return rc;
     if ((rc = make_map(c, enc, &c->tmM36, baseM, 4, FT_MW, FT_MH))) return rc;
     CK(cudaFuncSetAttribute(k_fused<FM_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
     CK(cudaFuncSetAttribute(k_fused<FM_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
@@ -589,9 +590,9 @@ static void fused_step(pact_ctx* c, Launcher& ln, int cur, float sgn, int kind)
         cudaStream_t s1 = both ? aux : st;
         const int grid = c->nwork[1];
         auto launch = [&] {
-            if (fa.P == 0) k_fused<FM_PLAIN><<<grid, FT_NT, FT_SMEM_BYTES, s1>>>(c->tmS40[cur], c->tmS36[cur], c->tmM40, c->tmM36, fb);
-            else if (sgn > 0.0f) k_fused<FM_FWD><<<grid, FT_NT, FT_SMEM_BYTES, s1>>>(c->tmS40[cur], c->tmS36[cur], c->tmM40, c->tmM36, fb);
-            else k_fused<FM_ADJ><<<grid, FT_NT, FT_SMEM_BYTES, s1>>>(c->tmS40[cur], c->tmS36[cur], c->tmM40, c->tmM36, fb);
+            if (fa.P == 0) k_fused<FM_PLAIN><<<grid, FT_NT, FT_SMEM_BYTES, s1>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, fb);
+            else if (sgn > 0.0f) k_fused<FM_FWD><<<grid, FT_NT, FT_SMEM_BYTES, s1>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, fb);
+            else k_fused<FM_ADJ><<<grid, FT_NT, FT_SMEM_BYTES, s1>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, fb);
         };
         if (both) { launch(); cudaEventRecord(c->ev_join, aux); }   // timed with the interior launch below (they overlap)
         else ln.run(kind, launch);
@@ -601,7 +602,7 @@ static void fused_step(pact_ctx* c, Launcher& ln, int cur, float sgn, int kind)
         fb.work = c->d_work[0];
         const int grid = c->nwork[0];
         ln.run(kind, [&] {
-            k_fused<FM_PLAIN><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM40, c->tmM36, fb);
+            k_fused<FM_PLAIN><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, fb);
             if (both) cudaStreamWaitEvent(st, c->ev_join, 0);
         });
     }
