@@ -259,7 +259,7 @@ def main():
     loop_f, k_f, n_f = ctx.timing("forward")
     loop_a, k_a, n_a = ctx.timing("adjoint")
     ctx.set_option("profile", 0)
-    launches = (sum(n_f.values()) + sum(n_a.values()) + 4) * args.steps   # + argument record x2, tau, tau^T per step
+    launches = (sum(n_f.values()) + sum(n_a.values()) + 3) * args.steps   # + argument record x2 and tau per step
     # device time of one time step's kernels (all launches of the step, in the mix they ran)
     t_fwd = (k_f["fwd_vel"] * n_f["fwd_vel"] + k_f["fwd_str"] * n_f["fwd_str"] + k_f["fwd_fused"] * n_f["fwd_fused"]) / max(prm.nt - 1, 1)
     t_adj = (k_a["adj_a"] * n_a["adj_a"] + k_a["adj_b"] * n_a["adj_b"] + k_a["adj_fused"] * n_a["adj_fused"]) / max(prm.nt - 1, 1)

@@ -129,12 +129,14 @@ int pact_set_option(pact_ctx* ctx, const char* key, long long value);
  */
 #define PACT_K_FWD_VEL   0   /* Eq. 46a,b */
 #define PACT_K_FWD_STR   1   /* Eq. 46c,d */
-#define PACT_K_FWD_FUSED 2   /* Eq. 46a-d in one pass */
+#define PACT_K_FWD_FUSED 2   /* Eq. 46a-d in one pass (interior launch + slab launch, timed as one) */
 #define PACT_K_ADJ_A     3   /* Eq. 61a,b,f : sigma_bar -> u_bar, psi_bar */
 #define PACT_K_ADJ_B     4   /* Eq. 61c,d,e,g : u_bar -> sigma_bar, phi_bar */
 #define PACT_K_ADJ_FUSED 5
 #define PACT_K_RECV      6   /* Theta gather / Theta^T scatter, Eq. 56, 60 */
-#define PACT_K_OTHER     7   /* tau, tau^T, argument record */
+#define PACT_K_OTHER     7   /* launches counted but not timed on their own: the C-PML (slab) launch of a fused
+                                step, which runs on a second stream beside the interior launch and is inside the
+                                PACT_K_*_FUSED time of that step */
 int pact_get_timing(pact_ctx* ctx, int op, double* loop_ms, double* kernel_ms, long long* launches);
 
 /* Bytes of device memory owned by the context. */

@@ -380,6 +380,9 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
     const bool pok = pml && act1 && x >= 0 && x < a.nxq && yin;     // quad has memory-variable storage (given z in range)
     const int colq = pok ? xslab_col(a, x) : -1;
     const int prow = pok ? yzslab_row(y, a.ny, a.P) : -1;
+    // adjoint: does any tap of this thread's differences along x / y fall into a slab
+    const bool nearx = pok && (colq >= 0 || xslab_col(a, x - 4) >= 0 || xslab_col(a, x + 4) >= 0);
+    const bool neary = pok && (y - 2 < a.P || y + 2 >= a.ny - 1 - a.P);
 
     const float* in = a.in;
     const long long box = a.box;
@@ -542,8 +545,8 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                     if (pz >= 0) t3 = pml_fwd_m(pm[2], a.mvo[2], idx_z(a, x, y, pz), ZT(T_A_INT)[kk & (FT_ZRING - 1)], ZT(T_B_INT)[kk & (FT_ZRING - 1)], t3, wr1);
                 }
                 if (MODE == FM_ADJ && pml1) {
-                    if (bx) { const Taps8 X = adj_x(a, a.mvi[9], a.mvo[9], XT(T_A_INT), XT(T_B_INT), x, y, kk, l, c11, rr, wr1); t1 = t1 + dpx(X.l, X.c, X.r); }
-                    if (by) t2 = t2 + adj_y(a, a.mvi[10], a.mvo[10], YT(T_A_HALF), YT(T_B_HALF), x, y - 2, kk, 2, ya, yb, c12, yd, wr1);
+                    if (nearx) { const Taps8 X = adj_x(a, a.mvi[9], a.mvo[9], XT(T_A_INT), XT(T_B_INT), x, y, kk, l, c11, rr, wr1); t1 = t1 + dpx(X.l, X.c, X.r); }
+                    if (neary) t2 = t2 + adj_y(a, a.mvi[10], a.mvo[10], YT(T_A_HALF), YT(T_B_HALF), x, y - 2, kk, 2, ya, yb, c12, yd, wr1);
                     if (bz) t3 = t3 + adj_z(a, a.mvi[11], a.mvo[11], ZT(T_A_HALF), ZT(T_B_HALF), x, y, kk - 2, 2, w13a, w13b, w13c, f13, wr1);
                 }
                 const float4 rxp = shl1(r0, PR[4 * uq + 4]), axp = shl1(a0, PA[4 * uq + 4]);
@@ -560,8 +563,8 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                     if (pz >= 0) t3 = pml_fwd_m(pm[5], a.mvo[5], idx_z(a, x, y, pz), ZT(T_A_INT)[kk & (FT_ZRING - 1)], ZT(T_B_INT)[kk & (FT_ZRING - 1)], t3, wr1);
                 }
                 if (MODE == FM_ADJ && pml1) {
-                    if (bx) { const Taps8 X = adj_x(a, a.mvi[12], a.mvo[12], XT(T_A_HALF), XT(T_B_HALF), x, y, kk, l, c12, rr, wr1); t1 = t1 + dmx(X.l, X.c, X.r); }
-                    if (by) t2 = t2 + adj_y(a, a.mvi[13], a.mvo[13], YT(T_A_INT), YT(T_B_INT), x, y - 1, kk, 1, yb, c22, yc, yd, wr1);
+                    if (nearx) { const Taps8 X = adj_x(a, a.mvi[12], a.mvo[12], XT(T_A_HALF), XT(T_B_HALF), x, y, kk, l, c12, rr, wr1); t1 = t1 + dmx(X.l, X.c, X.r); }
+                    if (neary) t2 = t2 + adj_y(a, a.mvi[13], a.mvo[13], YT(T_A_INT), YT(T_B_INT), x, y - 1, kk, 1, yb, c22, yc, yd, wr1);
                     if (bz) t3 = t3 + adj_z(a, a.mvi[14], a.mvo[14], ZT(T_A_HALF), ZT(T_B_HALF), x, y, kk - 2, 2, w23a, w23b, w23c, f23, wr1);
                 }
                 const float4 ryp = ld4s(PR, uq + 10), ayp = ld4s(PA, uq + 10);
@@ -577,8 +580,8 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                     if (pz >= 0) t3 = pml_fwd_m(pm[8], a.mvo[8], idx_z(a, x, y, pz), ZT(T_A_HALF)[kk & (FT_ZRING - 1)], ZT(T_B_HALF)[kk & (FT_ZRING - 1)], t3, wr1);
                 }
                 if (MODE == FM_ADJ && pml1) {
-                    if (bx) { const Taps8 X = adj_x(a, a.mvi[15], a.mvo[15], XT(T_A_HALF), XT(T_B_HALF), x, y, kk, l, w13c, rr, wr1); t1 = t1 + dmx(X.l, X.c, X.r); }
-                    if (by) t2 = t2 + adj_y(a, a.mvi[16], a.mvo[16], YT(T_A_HALF), YT(T_B_HALF), x, y - 2, kk, 2, ya, yb, w23c, yd, wr1);
+                    if (nearx) { const Taps8 X = adj_x(a, a.mvi[15], a.mvo[15], XT(T_A_HALF), XT(T_B_HALF), x, y, kk, l, w13c, rr, wr1); t1 = t1 + dmx(X.l, X.c, X.r); }
+                    if (neary) t2 = t2 + adj_y(a, a.mvi[16], a.mvo[16], YT(T_A_HALF), YT(T_B_HALF), x, y - 2, kk, 2, ya, yb, w23c, yd, wr1);
                     if (bz) t3 = t3 + adj_z(a, a.mvi[17], a.mvo[17], ZT(T_A_INT), ZT(T_B_INT), x, y, kk - 1, 1, w33b, w33c, w33d, f33, wr1);
                 }
                 const float4 rzp = ld4s(Rbase + s3n * FT_RPL, uq), azp = ld4s(Abase + s3n * FT_RPL, uq);
@@ -678,8 +681,8 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                     if (pz >= 0) g13 = pml_fwd_m(qm[2], a.mvo[11], idx_z(a, x, y, pz), ZT(T_A_HALF)[ks & (FT_ZRING - 1)], ZT(T_B_HALF)[ks & (FT_ZRING - 1)], g13, true);
                 }
                 if (MODE == FM_ADJ && pml2) {
-                    if (bx) { const Taps8 X = adj_x(a, a.mvi[0], nullptr, XT(T_A_HALF), XT(T_B_HALF), x, y, ks, l, c, rr, false); e11 = e11 + dmx(X.l, X.c, X.r); }
-                    if (by) g12 = g12 + adj_y(a, a.mvi[1], nullptr, YT(T_A_INT), YT(T_B_INT), x, y - 1, ks, 1, ya, c, yc, yd, false);
+                    if (nearx) { const Taps8 X = adj_x(a, a.mvi[0], nullptr, XT(T_A_HALF), XT(T_B_HALF), x, y, ks, l, c, rr, false); e11 = e11 + dmx(X.l, X.c, X.r); }
+                    if (neary) g12 = g12 + adj_y(a, a.mvi[1], nullptr, YT(T_A_INT), YT(T_B_INT), x, y - 1, ks, 1, ya, c, yc, yd, false);
                     if (bz) g13 = g13 + adj_z(a, a.mvi[2], nullptr, ZT(T_A_INT), ZT(T_B_INT), x, y, ks - 1, 1, za, c, zc, zd, false);
                 }
             }
@@ -695,8 +698,8 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                     if (pz >= 0) g23 = pml_fwd_m(qm[5], a.mvo[14], idx_z(a, x, y, pz), ZT(T_A_HALF)[ks & (FT_ZRING - 1)], ZT(T_B_HALF)[ks & (FT_ZRING - 1)], g23, true);
                 }
                 if (MODE == FM_ADJ && pml2) {
-                    if (bx) { const Taps8 X = adj_x(a, a.mvi[3], nullptr, XT(T_A_INT), XT(T_B_INT), x, y, ks, l, c, rr, false); g21 = g21 + dpx(X.l, X.c, X.r); }
-                    if (by) e22 = e22 + adj_y(a, a.mvi[4], nullptr, YT(T_A_HALF), YT(T_B_HALF), x, y - 2, ks, 2, ya, yb, c, yd, false);
+                    if (nearx) { const Taps8 X = adj_x(a, a.mvi[3], nullptr, XT(T_A_INT), XT(T_B_INT), x, y, ks, l, c, rr, false); g21 = g21 + dpx(X.l, X.c, X.r); }
+                    if (neary) e22 = e22 + adj_y(a, a.mvi[4], nullptr, YT(T_A_HALF), YT(T_B_HALF), x, y - 2, ks, 2, ya, yb, c, yd, false);
                     if (bz) g23 = g23 + adj_z(a, a.mvi[5], nullptr, ZT(T_A_INT), ZT(T_B_INT), x, y, ks - 1, 1, za, c, zc, zd, false);
                 }
             }
@@ -712,8 +715,8 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                     if (pz >= 0) e33 = pml_fwd_m(qm[8], a.mvo[17], idx_z(a, x, y, pz), ZT(T_A_INT)[ks & (FT_ZRING - 1)], ZT(T_B_INT)[ks & (FT_ZRING - 1)], e33, true);
                 }
                 if (MODE == FM_ADJ && pml2) {
-                    if (bx) { const Taps8 X = adj_x(a, a.mvi[6], nullptr, XT(T_A_INT), XT(T_B_INT), x, y, ks, l, c, rr, false); g31 = g31 + dpx(X.l, X.c, X.r); }
-                    if (by) g32 = g32 + adj_y(a, a.mvi[7], nullptr, YT(T_A_INT), YT(T_B_INT), x, y - 1, ks, 1, ya, c, yc, yd, false);
+                    if (nearx) { const Taps8 X = adj_x(a, a.mvi[6], nullptr, XT(T_A_INT), XT(T_B_INT), x, y, ks, l, c, rr, false); g31 = g31 + dpx(X.l, X.c, X.r); }
+                    if (neary) g32 = g32 + adj_y(a, a.mvi[7], nullptr, YT(T_A_INT), YT(T_B_INT), x, y - 1, ks, 1, ya, c, yc, yd, false);
                     if (bz) e33 = e33 + adj_z(a, a.mvi[8], nullptr, ZT(T_A_HALF), ZT(T_B_HALF), x, y, ks - 2, 2, za, zb_, c, zd, false);
                 }
             }

@@ -594,7 +594,11 @@ static void fused_step(pact_ctx* c, Launcher& ln, int cur, float sgn, int kind)
             else if (sgn > 0.0f) k_fused<FM_FWD><<<grid, FT_NT, FT_SMEM_BYTES, s1>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, fb);
             else k_fused<FM_ADJ><<<grid, FT_NT, FT_SMEM_BYTES, s1>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, fb);
         };
-        if (both) { launch(); cudaEventRecord(c->ev_join, aux); }   // timed with the interior launch below (they overlap)
+        if (both) {   // timed together with the interior launch below (they overlap); counted under PACT_K_OTHER
+            launch();
+            cudaEventRecord(c->ev_join, aux);
+            c->launches[ln.op][PACT_K_OTHER]++;
+        }
         else ln.run(kind, launch);
     }
     if (c->nwork[0] > 0) {
