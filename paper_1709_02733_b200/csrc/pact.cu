@@ -434,8 +434,10 @@ static int make_map(pact_ctx* c, encode_tiled_fn enc, CUtensorMap* tm, const flo
     const cuuint64_t strides[3] = {(cuuint64_t)c->pitch * 4, (cuuint64_t)c->pitch * c->py * 4, (cuuint64_t)c->box * 4};
     const cuuint32_t boxd[4] = {(cuuint32_t)bw, (cuuint32_t)bh, 1, 1};
     const cuuint32_t es[4] = {1, 1, 1, 1};
+    // L2 promotion 64 B: box rows are 160 B starting 112 B into a 128-B line; with 128-B promotion every row pulls
+    // three whole lines (measured: 12.0 GB of DRAM reads per 512^3 step against 9.5 GB with 64 B, 7.0 GB algorithmic)
     CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (void*)base, dims, strides, boxd, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                     CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                     CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_64B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         snprintf(g_cuda_err, sizeof(g_cuda_err), "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
         return PACT_ECUDA;
