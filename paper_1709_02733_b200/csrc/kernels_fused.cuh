@@ -45,7 +45,7 @@
 #define FT_RH 37                      // rows of the rho / alpha planes: u region + 1
 #define FT_RPL 1504                   // floats per rho / alpha plane buffer (40*37 = 1480, padded to 128 B)
 #define FT_LPL (FT_TX * FT_TY)        // floats per lambda plane (the tile itself)
-#define FT_RING 5                     // u planes in the ring: ks-1 .. ks+2 and the slot u_old(kk+1) is landing in
+#define FT_RING 4                     // u planes in the ring: ks .. ks+2 and the slot u_old(kk+1) is landing in
 
 // shared memory map (floats).  Planes are only as tall as their readers need: s11, s13 (x neighbours only) and
 // s33 (own column) cover the u region (36 rows), rho / alpha one row more, s22, s12, s23 the full 40.
@@ -59,7 +59,8 @@
 #define FT_OFF_S33 (FT_OFF_ALP + 3 * FT_RPL)
 #define FT_OFF_MU (FT_OFF_S33 + 2 * FT_UPL)
 #define FT_OFF_LAM (FT_OFF_MU + 3 * FT_MPL)
-#define FT_OFF_UR (FT_OFF_LAM + 2 * FT_LPL)
+#define FT_OFF_SO (FT_OFF_LAM + 2 * FT_LPL)       // old s11, s22 of plane ks (tile only): [slot][field]
+#define FT_OFF_UR (FT_OFF_SO + 4 * FT_LPL)
 #define FT_OFF_END (FT_OFF_UR + 3 * FT_RING * FT_UPL)
 #define FT_TABW 48                     // x / y C-PML table window: tile - 8 .. tile + 39
 #define FT_ZRING 16                   // z C-PML table ring (planes)
@@ -341,7 +342,7 @@ template <int MODE>
 __global__ void __launch_bounds__(FT_NT, 1)
 k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUtensorMap tmS36,
         const __grid_constant__ CUtensorMap tmM37, const __grid_constant__ CUtensorMap tmM36,
-        const __grid_constant__ CUtensorMap tmL, const FusedArgs a)
+        const __grid_constant__ CUtensorMap tmL, const __grid_constant__ CUtensorMap tmS32, const FusedArgs a)
 {
     extern __shared__ __align__(1024) float sm[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(sm + FT_OFF_END);
@@ -432,10 +433,13 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
     };
     auto issueM = [&](int j) {
         uint64_t* bar = &barM[j % 3];
-        mbar_expect_tx(bar, (FT_MW * FT_MH + FT_LPL) * 4);
+        mbar_expect_tx(bar, (FT_MW * FT_MH + 3 * FT_LPL) * 4);
         tma_plane(&tmM36, sm + FT_OFF_MU + (j % 3) * FT_MPL, bar, cxm, cym, cz0 + j, 1);
         // lambda of plane j - 1 (read by stage 2 of iteration j + 1, which waits on this barrier) -> slot (j - 1) & 1
         tma_plane(&tmL, sm + FT_OFF_LAM + ((j + 1) & 1) * FT_LPL, bar, cxm, cym, cz0 + j - 1, 0);
+        // and the old s11, s22 of that plane (the tile itself): they are the sigma(ks) that stage 2 adds to
+        tma_plane(&tmS32, sm + FT_OFF_SO + (2 * ((j + 1) & 1) + 0) * FT_LPL, bar, cxm, cym, cz0 + j - 1, S11);
+        tma_plane(&tmS32, sm + FT_OFF_SO + (2 * ((j + 1) & 1) + 1) * FT_LPL, bar, cxm, cym, cz0 + j - 1, S22);
     };
 
     // u_old(c) lands in the ring slot that u_new(c) will overwrite in place (own quads only)
@@ -453,8 +457,9 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
     float4 w13a, w13b, w13c;          // s13 at kk-2, kk-1, kk
     float4 w23a, w23b, w23c;          // s23
     float4 w33a, w33b, w33c, w33d;    // s33 at kk-2, kk-1, kk, kk+1
-    float4 u3m2 = f4(0.0f);           // u3(ks-2) of the thread's quad (its ring slot is refilled with u_old by then)
-    float4 so11, so22, so12;          // old s11, s22, s12 at ks = kk - 2
+    // own-quad z taps of stage 2 that are older than the ring: u(ks-1) and u3(ks-2) (their slots are being refilled)
+    float4 u1m1 = f4(0.0f), u2m1 = f4(0.0f), u3m1 = f4(0.0f), u3m2 = f4(0.0f);
+    float4 so12;                      // old s12 at ks = kk - 2 (the one own-column load left on the LSU path)
     const float4 z4 = f4(0.0f);
     {
         const long long g = (long long)(zb - 2) * a.sz + gxy;
@@ -468,7 +473,7 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
         w33b = ld_ok ? ldg4(in + S33 * box + g - a.sz) : z4;
         w33c = ld_ok ? ldg4(in + S33 * box + g) : z4;
         w33d = ld_ok ? ldg4(in + S33 * box + g + a.sz) : z4;
-        so11 = so22 = so12 = z4;
+        so12 = z4;
     }
 
     // coefficient scales: sign of the step and the 1/c2 of the unnormalised differences (d1)
@@ -655,25 +660,31 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
         if (it >= 1) mbar_wait(&barM[(it - 1) % 3], ((it - 1) / 3) & 1);
         // ------------------------------------------------------------------ stage 2: sigma(ks), ks = kk - 2
         const int ks = kk - 2;
-        // u3(ks-1) of the own quad; with u3m2 (the value read here one iteration ago) it replaces the two oldest ring planes
-        float4 u3m1 = z4;
-        if (inner && it >= 3) u3m1 = ld4s(sm + FT_OFF_UR + (2 * FT_RING + (it + 2) % FT_RING) * FT_UPL, uq);
+        // centre-plane values of the own quad: they become the (ks-1) taps of the next iteration (from it = 2 on, so
+        // that the first stage 2, at it = 4, finds u(ks-1) and u3(ks-2) in registers)
+        float4 cc1 = z4, cc2 = z4, cc3 = z4;
+        if (inner && it >= 2) {
+            const int pc = ((it + 2) % FT_RING) * FT_UPL;      // slot of plane it - 2
+            cc1 = ld4s(sm + FT_OFF_UR + 0 * FT_RING * FT_UPL + pc, uq);
+            cc2 = ld4s(sm + FT_OFF_UR + 1 * FT_RING * FT_UPL + pc, uq);
+            cc3 = ld4s(sm + FT_OFF_UR + 2 * FT_RING * FT_UPL + pc, uq);
+        }
         if (inner && it >= 4) {
             const int j = it - 2;             // relative plane of ks
             const float* U1p = sm + FT_OFF_UR + 0 * FT_RING * FT_UPL;
             const float* U2p = sm + FT_OFF_UR + 1 * FT_RING * FT_UPL;
             const float* U3p = sm + FT_OFF_UR + 2 * FT_RING * FT_UPL;
-            const int p0 = (j % FT_RING) * FT_UPL, pm1 = ((j + 4) % FT_RING) * FT_UPL;
+            const int p0 = (j % FT_RING) * FT_UPL;
             const int pp1 = ((j + 1) % FT_RING) * FT_UPL, pp2 = ((j + 2) % FT_RING) * FT_UPL;
             const int pz = pml ? yzslab_row(ks, a.nz, a.P) : -1;
             const bool bz = pml && (ks - 2 < a.P || ks + 2 >= a.nz - 1 - a.P);
             const bool pml2 = bx || by || bz;       // inner threads have storage: 0 <= x < nx, 0 <= y < ny, zb <= ks < ze
             float4 e11, e22, e33, g12, g21, g13, g31, g23, g32;
             {   // ---- derivatives of u1: D-x (e11), D+y (g12), D+z (g13)
-                const float4 c = ld4s(U1p + p0, uq);
+                const float4 c = cc1;
                 const float2 l = ld2s(U1p + p0, 4 * uq - 2), rr = ld2s(U1p + p0, 4 * uq + 4);
                 const float4 ya = ld4s(U1p + p0, uq - 10), yc = ld4s(U1p + p0, uq + 10), yd = ld4s(U1p + p0, uq + 20);
-                const float4 za = ld4s(U1p + pm1, uq), zc = ld4s(U1p + pp1, uq), zd = ld4s(U1p + pp2, uq);
+                const float4 za = u1m1, zc = ld4s(U1p + pp1, uq), zd = ld4s(U1p + pp2, uq);
                 e11 = dmx(l, c, rr); g12 = d4(ya, c, yc, yd); g13 = d4(za, c, zc, zd);
                 if (MODE == FM_FWD && pml2) {
                     if (colq >= 0) e11 = pml_fwd_m(qm[0], a.mvo[9], idx_x(a, colq, y, ks), tab4(XT(T_A_INT), x), tab4(XT(T_B_INT), x), e11, true);
@@ -687,10 +698,10 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                 }
             }
             {   // ---- derivatives of u2: D+x (g21), D-y (e22), D+z (g23)
-                const float4 c = ld4s(U2p + p0, uq);
+                const float4 c = cc2;
                 const float2 l = ld2s(U2p + p0, 4 * uq - 2), rr = ld2s(U2p + p0, 4 * uq + 4);
                 const float4 ya = ld4s(U2p + p0, uq - 20), yb = ld4s(U2p + p0, uq - 10), yd = ld4s(U2p + p0, uq + 10);
-                const float4 za = ld4s(U2p + pm1, uq), zc = ld4s(U2p + pp1, uq), zd = ld4s(U2p + pp2, uq);
+                const float4 za = u2m1, zc = ld4s(U2p + pp1, uq), zd = ld4s(U2p + pp2, uq);
                 g21 = dpx(l, c, rr); e22 = d4(ya, yb, c, yd); g23 = d4(za, c, zc, zd);
                 if (MODE == FM_FWD && pml2) {
                     if (colq >= 0) g21 = pml_fwd_m(qm[3], a.mvo[12], idx_x(a, colq, y, ks), tab4(XT(T_A_HALF), x), tab4(XT(T_B_HALF), x), g21, true);
@@ -704,7 +715,7 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                 }
             }
             {   // ---- derivatives of u3: D+x (g31), D+y (g32), D-z (e33)
-                const float4 c = ld4s(U3p + p0, uq);
+                const float4 c = cc3;
                 const float2 l = ld2s(U3p + p0, 4 * uq - 2), rr = ld2s(U3p + p0, 4 * uq + 4);
                 const float4 ya = ld4s(U3p + p0, uq - 10), yc = ld4s(U3p + p0, uq + 10), yd = ld4s(U3p + p0, uq + 20);
                 const float4 za = u3m2, zb_ = u3m1, zd = ld4s(U3p + pp1, uq);
@@ -732,8 +743,9 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
             const float4 myz = kM * rcp4((i0 + iy) + (iz + iyz));
             const float4 lam = ld4s(sm + FT_OFF_LAM + (it & 1) * FT_LPL, (r - 2) * 8 + (qx - 1));   // lambda(ks), by TMA
             const float4 ldiv = (kL * lam) * (e11 + e22 + e33);
-            const float4 n11 = so11 + fma4(mn2, e11, ldiv);
-            const float4 n22 = so22 + fma4(mn2, e22, ldiv);
+            const int lq = (r - 2) * 8 + (qx - 1);
+            const float4 n11 = ld4s(sm + FT_OFF_SO + (2 * (it & 1) + 0) * FT_LPL, lq) + fma4(mn2, e11, ldiv);
+            const float4 n22 = ld4s(sm + FT_OFF_SO + (2 * (it & 1) + 1) * FT_LPL, lq) + fma4(mn2, e22, ldiv);
             const float4 n33 = w33a + fma4(mn2, e33, ldiv);
             const float4 n12 = fma4(mxy, g12 + g21, so12);
             const float4 n13 = fma4(mxz, g13 + g31, w13a);
@@ -749,11 +761,9 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
         {   // own-column inputs of the next stage 2 (plane ks + 1)
             const bool p = inner && it >= 3 && it + 1 < itn;
             const long long g = (long long)(ks + 1) * a.sz + gxy;
-            ldg4_into(so11, in + S11 * box + g, p);
-            ldg4_into(so22, in + S22 * box + g, p);
             ldg4_into(so12, in + S12 * box + g, p);
         }
-        u3m2 = u3m1;
+        u3m2 = u3m1; u1m1 = cc1; u2m1 = cc2; u3m1 = cc3;
         // slide the z windows
         w13a = w13b; w13b = w13c; w13c = f13;
         w23a = w23b; w23b = w23c; w23c = f23;

@@ -63,7 +63,7 @@ struct pact_ctx {
     DevGrid g2;              // view of state buffer B for the I/O kernels
     float* stateB_base;
     long long stateB_bytes;
-    CUtensorMap tmS40[2], tmS36[2], tmM37, tmM36, tmL;
+    CUtensorMap tmS40[2], tmS36[2], tmS32[2], tmM37, tmM36, tmL;
     FusedArgs fa;
     int zchunk;              // planes per CTA along z (0 = auto)
     // work lists of the fused launches: [0] CTAs whose bricks (with every tap of the adjoint) stay clear of the
@@ -500,6 +500,8 @@ static int ensure_fused(pact_ctx* c)
     if ((rc = make_map(c, enc, &c->tmS40[0], baseA, NFIELD, FT_BW, FT_BH))) return rc;
     if ((rc = make_map(c, enc, &c->tmS36[0], baseA, NFIELD, FT_BW, FT_UH))) return rc;
     if ((rc = make_map(c, enc, &c->tmS40[1], baseB, NFIELD, FT_BW, FT_BH))) return rc;
+    if ((rc = make_map(c, enc, &c->tmS32[0], baseA, NFIELD, FT_TX, FT_TY))) return rc;
+    if ((rc = make_map(c, enc, &c->tmS32[1], baseB, NFIELD, FT_TX, FT_TY))) return rc;
     if ((rc = make_map(c, enc, &c->tmS36[1], baseB, NFIELD, FT_BW, FT_UH))) return rc;
     if ((rc = make_map(c, enc, &c->tmM37, baseM, 4, FT_BW, FT_RH))) return rc;
     if ((rc = make_map(c, enc, &c->tmL, baseM, 4, FT_TX, FT_TY))) return rc;
@@ -592,9 +594,9 @@ static void fused_step(pact_ctx* c, Launcher& ln, int cur, float sgn, int kind)
         cudaStream_t s1 = both ? aux : st;
         const int grid = c->nwork[1];
         auto launch = [&] {
-            if (fa.P == 0) k_fused<FM_PLAIN><<<grid, FT_NT, FT_SMEM_BYTES, s1>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, fb);
-            else if (sgn > 0.0f) k_fused<FM_FWD><<<grid, FT_NT, FT_SMEM_BYTES, s1>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, fb);
-            else k_fused<FM_ADJ><<<grid, FT_NT, FT_SMEM_BYTES, s1>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, fb);
+            if (fa.P == 0) k_fused<FM_PLAIN><<<grid, FT_NT, FT_SMEM_BYTES, s1>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fb);
+            else if (sgn > 0.0f) k_fused<FM_FWD><<<grid, FT_NT, FT_SMEM_BYTES, s1>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fb);
+            else k_fused<FM_ADJ><<<grid, FT_NT, FT_SMEM_BYTES, s1>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fb);
         };
         if (both) {   // timed together with the interior launch below (they overlap); counted under PACT_K_OTHER
             launch();
@@ -608,7 +610,7 @@ static void fused_step(pact_ctx* c, Launcher& ln, int cur, float sgn, int kind)
         fb.work = c->d_work[0];
         const int grid = c->nwork[0];
         ln.run(kind, [&] {
-            k_fused<FM_PLAIN><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, fb);
+            k_fused<FM_PLAIN><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fb);
             if (both) cudaStreamWaitEvent(st, c->ev_join, 0);
         });
     }
