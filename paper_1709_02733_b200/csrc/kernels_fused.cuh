@@ -459,7 +459,6 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
     float4 w33a, w33b, w33c, w33d;    // s33 at kk-2, kk-1, kk, kk+1
     // own-quad z taps of stage 2 that are older than the ring: u(ks-1) and u3(ks-2) (their slots are being refilled)
     float4 u1m1 = f4(0.0f), u2m1 = f4(0.0f), u3m1 = f4(0.0f), u3m2 = f4(0.0f);
-    float4 so12;                      // old s12 at ks = kk - 2 (the one own-column load left on the LSU path)
     const float4 z4 = f4(0.0f);
     {
         const long long g = (long long)(zb - 2) * a.sz + gxy;
@@ -473,7 +472,6 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
         w33b = ld_ok ? ldg4(in + S33 * box + g - a.sz) : z4;
         w33c = ld_ok ? ldg4(in + S33 * box + g) : z4;
         w33d = ld_ok ? ldg4(in + S33 * box + g + a.sz) : z4;
-        so12 = z4;
     }
 
     // coefficient scales: sign of the step and the 1/c2 of the unnormalised differences (d1)
@@ -671,6 +669,10 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
         }
         if (inner && it >= 4) {
             const int j = it - 2;             // relative plane of ks
+            // old s12(ks): the one own-column load left on the LSU path (an L2 hit: group ks fetched the plane two
+            // iterations ago).  Issued here and consumed at the end of the stage: a load in flight across the loop
+            // back-edge makes ptxas wait for it at the loop head, every iteration.
+            const float4 so12 = ldg4(in + S12 * box + (long long)ks * a.sz + gxy);
             const float* U1p = sm + FT_OFF_UR + 0 * FT_RING * FT_UPL;
             const float* U2p = sm + FT_OFF_UR + 1 * FT_RING * FT_UPL;
             const float* U3p = sm + FT_OFF_UR + 2 * FT_RING * FT_UPL;
@@ -757,11 +759,6 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
             store_quad(a.out + S12 * box + g, n12, x, a.nx);
             store_quad(a.out + S13 * box + g, n13, x, a.nx);
             store_quad(a.out + S23 * box + g, n23, x, a.nx);
-        }
-        {   // own-column inputs of the next stage 2 (plane ks + 1)
-            const bool p = inner && it >= 3 && it + 1 < itn;
-            const long long g = (long long)(ks + 1) * a.sz + gxy;
-            ldg4_into(so12, in + S12 * box + g, p);
         }
         u3m2 = u3m1; u1m1 = cc1; u2m1 = cc2; u3m1 = cc3;
         // slide the z windows
