@@ -330,6 +330,26 @@ __device__ __forceinline__ float4 adj_z(const FusedArgs& a, const float* __restr
     }
     return d4(X[0], X[1], X[2], X[3]);
 }
+// Own-quad part of the same: T <- b T + s (stored by the owner) ; returns X = a T, zero outside the slab.  Used when
+// the CTA exchanges X through shared memory instead of re-deriving the neighbours' values (one slab axis per CTA).
+__device__ __forceinline__ float4 adj_x_own(const FusedArgs& a, const float* __restrict__ Ti, float* __restrict__ To,
+                                            const float* ta, const float* tb, int x, int y, int z, int col, float4 s, bool wr)
+{
+    if (col < 0) return f4(0.0f);
+    const long long i = idx_x(a, col, y, z);
+    const float4 Tn = fma4(tab4(tb, x), ldg4(Ti + i), s);
+    if (wr) stg4(To + i, Tn);
+    return tab4(ta, x) * Tn;
+}
+__device__ __forceinline__ float4 adj_y_own(const FusedArgs& a, const float* __restrict__ Ti, float* __restrict__ To,
+                                            const float* ta, const float* tb, int x, int y, int z, int row, float4 s, bool wr)
+{
+    if (row < 0) return f4(0.0f);
+    const long long i = idx_y(a, x, row, z);
+    const float4 Tn = fma4(tb[y], ldg4(Ti + i), s);
+    if (wr) stg4(To + i, Tn);
+    return ta[y] * Tn;
+}
 // tilde-form update of an own-quad memory variable fed by the new value v: T <- b T + v
 __device__ __forceinline__ void adj_own(const float* Ti, float* To, long long i, float4 b4, float4 v) { stg4(To + i, fma4(b4, ldg4(Ti + i), v)); }
 __device__ __forceinline__ void adj_own(const float* Ti, float* To, long long i, float b1, float4 v) { stg4(To + i, fma4(b1, ldg4(Ti + i), v)); }
@@ -384,6 +404,10 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
     // adjoint: does any tap of this thread's differences along x / y fall into a slab
     const bool nearx = pok && (colq >= 0 || xslab_col(a, x - 4) >= 0 || xslab_col(a, x + 4) >= 0);
     const bool neary = pok && (y - 2 < a.P || y + 2 >= a.ny - 1 - a.P);
+
+    // adjoint: slab axis whose filtered taps this CTA exchanges through shared memory (x if it touches the x slabs,
+    // else y), -1 = none.  CTA-uniform: it adds block barriers.
+    const int exa = (MODE == FM_ADJ) ? (bx ? 0 : (by ? 1 : -1)) : -1;
 
     const float* in = a.in;
     const long long box = a.box;
@@ -510,6 +534,36 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
         float4 f13 = z4, f23 = z4, f33 = z4;     // fresh window entries: s13, s23 at kk+1, s33 at kk+2
         const bool zin = (unsigned)kk < (unsigned)a.nz;
         // ------------------------------------------------------------------ stage 1: u(kk)
+        // Adjoint slab CTAs: X = a T of the own quad for the three terms of the exchange axis, T <- b T + s, into the ring
+        // slot that u_old(kk+1) will land in after the barrier (free: the closing barrier of the previous iteration's
+        // stage 2 was passed by every thread).
+        float* const SC1 = sm + FT_OFF_UR + ((it + 1) % FT_RING) * FT_UPL;     // + f * FT_RING * FT_UPL
+        if (exa >= 0) {
+            if (act1) {
+                float4 X0 = z4, X1 = z4, X2 = z4;
+                if (pok && zin) {
+                    const bool wr = inner && kk >= zb && kk < ze;
+                    const float4 o12 = ld4s(sm + FT_OFF_S12 + (it & 1) * FT_BOX, q);
+                    if (exa == 0) {
+                        const float4 o11 = ld4s(sm + FT_OFF_S11 + (it & 1) * FT_UPL, uq);
+                        X0 = adj_x_own(a, a.mvi[9], a.mvo[9], XT(T_A_INT), XT(T_B_INT), x, y, kk, colq, o11, wr);
+                        X1 = adj_x_own(a, a.mvi[12], a.mvo[12], XT(T_A_HALF), XT(T_B_HALF), x, y, kk, colq, o12, wr);
+                        X2 = adj_x_own(a, a.mvi[15], a.mvo[15], XT(T_A_HALF), XT(T_B_HALF), x, y, kk, colq, w13c, wr);
+                    } else {
+                        const float4 o22 = ld4s(sm + FT_OFF_S22 + (it & 1) * FT_BOX, q);
+                        X0 = adj_y_own(a, a.mvi[10], a.mvo[10], YT(T_A_HALF), YT(T_B_HALF), x, y, kk, prow, o12, wr);
+                        X1 = adj_y_own(a, a.mvi[13], a.mvo[13], YT(T_A_INT), YT(T_B_INT), x, y, kk, prow, o22, wr);
+                        X2 = adj_y_own(a, a.mvi[16], a.mvo[16], YT(T_A_HALF), YT(T_B_HALF), x, y, kk, prow, w23c, wr);
+                    }
+                }
+                *reinterpret_cast<float4*>(SC1 + 0 * FT_RING * FT_UPL + 4 * uq) = X0;
+                *reinterpret_cast<float4*>(SC1 + 1 * FT_RING * FT_UPL + 4 * uq) = X1;
+                *reinterpret_cast<float4*>(SC1 + 2 * FT_RING * FT_UPL + 4 * uq) = X2;
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // TMA overwrites these planes later
+            }
+            __syncthreads();
+        }
+        const bool yex = exa == 1 && r >= 2 && r < 34;      // all four y taps of this thread lie in the exchanged region
         if (act1) {
             const float* P11 = sm + FT_OFF_S11 + (it & 1) * FT_UPL;
             const float* P22 = sm + FT_OFF_S22 + (it & 1) * FT_BOX;
@@ -548,8 +602,11 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                     if (pz >= 0) t3 = pml_fwd_m(pm[2], a.mvo[2], idx_z(a, x, y, pz), ZT(T_A_INT)[kk & (FT_ZRING - 1)], ZT(T_B_INT)[kk & (FT_ZRING - 1)], t3, wr1);
                 }
                 if (MODE == FM_ADJ && pml1) {
-                    if (nearx) { const Taps8 X = adj_x(a, a.mvi[9], a.mvo[9], XT(T_A_INT), XT(T_B_INT), x, y, kk, l, c11, rr, wr1); t1 = t1 + dpx(X.l, X.c, X.r); }
-                    if (neary) t2 = t2 + adj_y(a, a.mvi[10], a.mvo[10], YT(T_A_HALF), YT(T_B_HALF), x, y - 2, kk, 2, ya, yb, c12, yd, wr1);
+                    const float* S = SC1 + 0 * FT_RING * FT_UPL;
+                    if (exa == 0) t1 = t1 + dpx(ld2s(S, 4 * uq - 2), ld4s(S, uq), ld2s(S, 4 * uq + 4));
+                    else if (nearx) { const Taps8 X = adj_x(a, a.mvi[9], a.mvo[9], XT(T_A_INT), XT(T_B_INT), x, y, kk, l, c11, rr, wr1); t1 = t1 + dpx(X.l, X.c, X.r); }
+                    if (yex) t2 = t2 + d4(ld4s(S, uq - 20), ld4s(S, uq - 10), ld4s(S, uq), ld4s(S, uq + 10));
+                    else if (neary) t2 = t2 + adj_y(a, a.mvi[10], a.mvo[10], YT(T_A_HALF), YT(T_B_HALF), x, y - 2, kk, 2, ya, yb, c12, yd, wr1 && exa != 1);
                     if (bz) t3 = t3 + adj_z(a, a.mvi[11], a.mvo[11], ZT(T_A_HALF), ZT(T_B_HALF), x, y, kk - 2, 2, w13a, w13b, w13c, f13, wr1);
                 }
                 const float4 rxp = shl1(r0, PR[4 * uq + 4]), axp = shl1(a0, PA[4 * uq + 4]);
@@ -566,8 +623,11 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                     if (pz >= 0) t3 = pml_fwd_m(pm[5], a.mvo[5], idx_z(a, x, y, pz), ZT(T_A_INT)[kk & (FT_ZRING - 1)], ZT(T_B_INT)[kk & (FT_ZRING - 1)], t3, wr1);
                 }
                 if (MODE == FM_ADJ && pml1) {
-                    if (nearx) { const Taps8 X = adj_x(a, a.mvi[12], a.mvo[12], XT(T_A_HALF), XT(T_B_HALF), x, y, kk, l, c12, rr, wr1); t1 = t1 + dmx(X.l, X.c, X.r); }
-                    if (neary) t2 = t2 + adj_y(a, a.mvi[13], a.mvo[13], YT(T_A_INT), YT(T_B_INT), x, y - 1, kk, 1, yb, c22, yc, yd, wr1);
+                    const float* S = SC1 + 1 * FT_RING * FT_UPL;
+                    if (exa == 0) t1 = t1 + dmx(ld2s(S, 4 * uq - 2), ld4s(S, uq), ld2s(S, 4 * uq + 4));
+                    else if (nearx) { const Taps8 X = adj_x(a, a.mvi[12], a.mvo[12], XT(T_A_HALF), XT(T_B_HALF), x, y, kk, l, c12, rr, wr1); t1 = t1 + dmx(X.l, X.c, X.r); }
+                    if (yex) t2 = t2 + d4(ld4s(S, uq - 10), ld4s(S, uq), ld4s(S, uq + 10), ld4s(S, uq + 20));
+                    else if (neary) t2 = t2 + adj_y(a, a.mvi[13], a.mvo[13], YT(T_A_INT), YT(T_B_INT), x, y - 1, kk, 1, yb, c22, yc, yd, wr1 && exa != 1);
                     if (bz) t3 = t3 + adj_z(a, a.mvi[14], a.mvo[14], ZT(T_A_HALF), ZT(T_B_HALF), x, y, kk - 2, 2, w23a, w23b, w23c, f23, wr1);
                 }
                 const float4 ryp = ld4s(PR, uq + 10), ayp = ld4s(PA, uq + 10);
@@ -583,8 +643,11 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                     if (pz >= 0) t3 = pml_fwd_m(pm[8], a.mvo[8], idx_z(a, x, y, pz), ZT(T_A_HALF)[kk & (FT_ZRING - 1)], ZT(T_B_HALF)[kk & (FT_ZRING - 1)], t3, wr1);
                 }
                 if (MODE == FM_ADJ && pml1) {
-                    if (nearx) { const Taps8 X = adj_x(a, a.mvi[15], a.mvo[15], XT(T_A_HALF), XT(T_B_HALF), x, y, kk, l, w13c, rr, wr1); t1 = t1 + dmx(X.l, X.c, X.r); }
-                    if (neary) t2 = t2 + adj_y(a, a.mvi[16], a.mvo[16], YT(T_A_HALF), YT(T_B_HALF), x, y - 2, kk, 2, ya, yb, w23c, yd, wr1);
+                    const float* S = SC1 + 2 * FT_RING * FT_UPL;
+                    if (exa == 0) t1 = t1 + dmx(ld2s(S, 4 * uq - 2), ld4s(S, uq), ld2s(S, 4 * uq + 4));
+                    else if (nearx) { const Taps8 X = adj_x(a, a.mvi[15], a.mvo[15], XT(T_A_HALF), XT(T_B_HALF), x, y, kk, l, w13c, rr, wr1); t1 = t1 + dmx(X.l, X.c, X.r); }
+                    if (yex) t2 = t2 + d4(ld4s(S, uq - 20), ld4s(S, uq - 10), ld4s(S, uq), ld4s(S, uq + 10));
+                    else if (neary) t2 = t2 + adj_y(a, a.mvi[16], a.mvo[16], YT(T_A_HALF), YT(T_B_HALF), x, y - 2, kk, 2, ya, yb, w23c, yd, wr1 && exa != 1);
                     if (bz) t3 = t3 + adj_z(a, a.mvi[17], a.mvo[17], ZT(T_A_INT), ZT(T_B_INT), x, y, kk - 1, 1, w33b, w33c, w33d, f33, wr1);
                 }
                 const float4 rzp = ld4s(Rbase + s3n * FT_RPL, uq), azp = ld4s(Abase + s3n * FT_RPL, uq);
@@ -653,7 +716,7 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
         if (tid == 0) {
             if (it + 1 < itn) issueU(it + 1);   // needed first ; slot of plane it - 4: its last cross-thread reads were in stage 2 of it - 2
             if (it + 2 <= itn) issueM(it);
-            if (it + 2 < itn) issueG(it + 2);
+            if (exa < 0 && it + 2 < itn) issueG(it + 2);   // exchange CTAs: after stage 2 (its slots are their scratch)
         }
         if (it >= 1) mbar_wait(&barM[(it - 1) % 3], ((it - 1) / 3) & 1);
         // ------------------------------------------------------------------ stage 2: sigma(ks), ks = kk - 2
@@ -666,6 +729,36 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
             cc1 = ld4s(sm + FT_OFF_UR + 0 * FT_RING * FT_UPL + pc, uq);
             cc2 = ld4s(sm + FT_OFF_UR + 1 * FT_RING * FT_UPL + pc, uq);
             cc3 = ld4s(sm + FT_OFF_UR + 2 * FT_RING * FT_UPL + pc, uq);
+        }
+        // Adjoint slab CTAs: Y = a T' of the own quad (T' = b T'_old + u_bar(ks), not stored here: stage 1 of plane ks did)
+        // for the three terms of the exchange axis, into the s22 / s12 / s11 planes that stage 1 has finished with.
+        float* const SC2a = sm + FT_OFF_S22 + (it & 1) * FT_BOX;
+        float* const SC2b = sm + FT_OFF_S12 + (it & 1) * FT_BOX;
+        float* const SC2c = sm + FT_OFF_S11 + (it & 1) * FT_UPL;
+        if (exa >= 0) {
+            if (act1 && it >= 4) {
+                float4 Y0 = z4, Y1 = z4, Y2 = z4;
+                if (pok && (unsigned)ks < (unsigned)a.nz) {
+                    const int pc = ((it + 2) % FT_RING) * FT_UPL;      // slot of the centre plane it - 2
+                    const float4 v1 = ld4s(sm + FT_OFF_UR + 0 * FT_RING * FT_UPL + pc, uq);
+                    const float4 v2 = ld4s(sm + FT_OFF_UR + 1 * FT_RING * FT_UPL + pc, uq);
+                    const float4 v3 = ld4s(sm + FT_OFF_UR + 2 * FT_RING * FT_UPL + pc, uq);
+                    if (exa == 0) {
+                        Y0 = adj_x_own(a, a.mvi[0], nullptr, XT(T_A_HALF), XT(T_B_HALF), x, y, ks, colq, v1, false);
+                        Y1 = adj_x_own(a, a.mvi[3], nullptr, XT(T_A_INT), XT(T_B_INT), x, y, ks, colq, v2, false);
+                        Y2 = adj_x_own(a, a.mvi[6], nullptr, XT(T_A_INT), XT(T_B_INT), x, y, ks, colq, v3, false);
+                    } else {
+                        Y0 = adj_y_own(a, a.mvi[1], nullptr, YT(T_A_INT), YT(T_B_INT), x, y, ks, prow, v1, false);
+                        Y1 = adj_y_own(a, a.mvi[4], nullptr, YT(T_A_HALF), YT(T_B_HALF), x, y, ks, prow, v2, false);
+                        Y2 = adj_y_own(a, a.mvi[7], nullptr, YT(T_A_INT), YT(T_B_INT), x, y, ks, prow, v3, false);
+                    }
+                }
+                *reinterpret_cast<float4*>(SC2a + 4 * uq) = Y0;
+                *reinterpret_cast<float4*>(SC2b + 4 * uq) = Y1;
+                *reinterpret_cast<float4*>(SC2c + 4 * uq) = Y2;
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            }
+            __syncthreads();
         }
         if (inner && it >= 4) {
             const int j = it - 2;             // relative plane of ks
@@ -694,8 +787,10 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                     if (pz >= 0) g13 = pml_fwd_m(qm[2], a.mvo[11], idx_z(a, x, y, pz), ZT(T_A_HALF)[ks & (FT_ZRING - 1)], ZT(T_B_HALF)[ks & (FT_ZRING - 1)], g13, true);
                 }
                 if (MODE == FM_ADJ && pml2) {
-                    if (nearx) { const Taps8 X = adj_x(a, a.mvi[0], nullptr, XT(T_A_HALF), XT(T_B_HALF), x, y, ks, l, c, rr, false); e11 = e11 + dmx(X.l, X.c, X.r); }
-                    if (neary) g12 = g12 + adj_y(a, a.mvi[1], nullptr, YT(T_A_INT), YT(T_B_INT), x, y - 1, ks, 1, ya, c, yc, yd, false);
+                    if (exa == 0) e11 = e11 + dmx(ld2s(SC2a, 4 * uq - 2), ld4s(SC2a, uq), ld2s(SC2a, 4 * uq + 4));
+                    else if (nearx) { const Taps8 X = adj_x(a, a.mvi[0], nullptr, XT(T_A_HALF), XT(T_B_HALF), x, y, ks, l, c, rr, false); e11 = e11 + dmx(X.l, X.c, X.r); }
+                    if (exa == 1) g12 = g12 + d4(ld4s(SC2a, uq - 10), ld4s(SC2a, uq), ld4s(SC2a, uq + 10), ld4s(SC2a, uq + 20));
+                    else if (neary) g12 = g12 + adj_y(a, a.mvi[1], nullptr, YT(T_A_INT), YT(T_B_INT), x, y - 1, ks, 1, ya, c, yc, yd, false);
                     if (bz) g13 = g13 + adj_z(a, a.mvi[2], nullptr, ZT(T_A_INT), ZT(T_B_INT), x, y, ks - 1, 1, za, c, zc, zd, false);
                 }
             }
@@ -711,8 +806,10 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                     if (pz >= 0) g23 = pml_fwd_m(qm[5], a.mvo[14], idx_z(a, x, y, pz), ZT(T_A_HALF)[ks & (FT_ZRING - 1)], ZT(T_B_HALF)[ks & (FT_ZRING - 1)], g23, true);
                 }
                 if (MODE == FM_ADJ && pml2) {
-                    if (nearx) { const Taps8 X = adj_x(a, a.mvi[3], nullptr, XT(T_A_INT), XT(T_B_INT), x, y, ks, l, c, rr, false); g21 = g21 + dpx(X.l, X.c, X.r); }
-                    if (neary) e22 = e22 + adj_y(a, a.mvi[4], nullptr, YT(T_A_HALF), YT(T_B_HALF), x, y - 2, ks, 2, ya, yb, c, yd, false);
+                    if (exa == 0) g21 = g21 + dpx(ld2s(SC2b, 4 * uq - 2), ld4s(SC2b, uq), ld2s(SC2b, 4 * uq + 4));
+                    else if (nearx) { const Taps8 X = adj_x(a, a.mvi[3], nullptr, XT(T_A_INT), XT(T_B_INT), x, y, ks, l, c, rr, false); g21 = g21 + dpx(X.l, X.c, X.r); }
+                    if (exa == 1) e22 = e22 + d4(ld4s(SC2b, uq - 20), ld4s(SC2b, uq - 10), ld4s(SC2b, uq), ld4s(SC2b, uq + 10));
+                    else if (neary) e22 = e22 + adj_y(a, a.mvi[4], nullptr, YT(T_A_HALF), YT(T_B_HALF), x, y - 2, ks, 2, ya, yb, c, yd, false);
                     if (bz) g23 = g23 + adj_z(a, a.mvi[5], nullptr, ZT(T_A_INT), ZT(T_B_INT), x, y, ks - 1, 1, za, c, zc, zd, false);
                 }
             }
@@ -728,8 +825,10 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                     if (pz >= 0) e33 = pml_fwd_m(qm[8], a.mvo[17], idx_z(a, x, y, pz), ZT(T_A_INT)[ks & (FT_ZRING - 1)], ZT(T_B_INT)[ks & (FT_ZRING - 1)], e33, true);
                 }
                 if (MODE == FM_ADJ && pml2) {
-                    if (nearx) { const Taps8 X = adj_x(a, a.mvi[6], nullptr, XT(T_A_INT), XT(T_B_INT), x, y, ks, l, c, rr, false); g31 = g31 + dpx(X.l, X.c, X.r); }
-                    if (neary) g32 = g32 + adj_y(a, a.mvi[7], nullptr, YT(T_A_INT), YT(T_B_INT), x, y - 1, ks, 1, ya, c, yc, yd, false);
+                    if (exa == 0) g31 = g31 + dpx(ld2s(SC2c, 4 * uq - 2), ld4s(SC2c, uq), ld2s(SC2c, 4 * uq + 4));
+                    else if (nearx) { const Taps8 X = adj_x(a, a.mvi[6], nullptr, XT(T_A_INT), XT(T_B_INT), x, y, ks, l, c, rr, false); g31 = g31 + dpx(X.l, X.c, X.r); }
+                    if (exa == 1) g32 = g32 + d4(ld4s(SC2c, uq - 10), ld4s(SC2c, uq), ld4s(SC2c, uq + 10), ld4s(SC2c, uq + 20));
+                    else if (neary) g32 = g32 + adj_y(a, a.mvi[7], nullptr, YT(T_A_INT), YT(T_B_INT), x, y - 1, ks, 1, ya, c, yc, yd, false);
                     if (bz) e33 = e33 + adj_z(a, a.mvi[8], nullptr, ZT(T_A_HALF), ZT(T_B_HALF), x, y, ks - 2, 2, za, zb_, c, zd, false);
                 }
             }
@@ -759,6 +858,10 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
             store_quad(a.out + S12 * box + g, n12, x, a.nx);
             store_quad(a.out + S13 * box + g, n13, x, a.nx);
             store_quad(a.out + S23 * box + g, n23, x, a.nx);
+        }
+        if (exa >= 0) {   // every thread is done with the exchange planes: now the group that refills them may go
+            __syncthreads();
+            if (tid == 0 && it + 2 < itn) issueG(it + 2);
         }
         u3m2 = u3m1; u1m1 = cc1; u2m1 = cc2; u3m1 = cc3;
         // slide the z windows
