@@ -350,6 +350,14 @@ __device__ __forceinline__ float4 adj_y_own(const FusedArgs& a, const float* __r
     if (wr) stg4(To + i, Tn);
     return ta[y] * Tn;
 }
+// the same with the old T already in registers (loaded ahead of a barrier)
+__device__ __forceinline__ float4 adj_own_x(float4 Told, float* To, long long i, bool in_slab, float4 a4, float4 b4, float4 s, bool wr)
+{
+    if (!in_slab) return f4(0.0f);
+    const float4 Tn = fma4(b4, Told, s);
+    if (wr) stg4(To + i, Tn);
+    return a4 * Tn;
+}
 // tilde-form update of an own-quad memory variable fed by the new value v: T <- b T + v
 __device__ __forceinline__ void adj_own(const float* Ti, float* To, long long i, float4 b4, float4 v) { stg4(To + i, fma4(b4, ldg4(Ti + i), v)); }
 __device__ __forceinline__ void adj_own(const float* Ti, float* To, long long i, float b1, float4 v) { stg4(To + i, fma4(b1, ldg4(Ti + i), v)); }
@@ -528,6 +536,20 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                 ldg4_into(pm[2], a.mvi[2] + iz, ez); ldg4_into(pm[5], a.mvi[5] + iz, ez); ldg4_into(pm[8], a.mvi[8] + iz, ez);
             }
         }
+        // adjoint exchange CTAs: the three old T of the own quad (plane kk) for the pre-block of stage 1, issued ahead
+        float4 e1[3];
+        long long ie1 = 0;
+        bool se1 = false;
+        if (MODE == FM_ADJ) {
+            e1[0] = e1[1] = e1[2] = f4(0.0f);
+            if (exa >= 0) {
+                const bool ok = pok && (unsigned)kk < (unsigned)a.nz;
+                se1 = ok && (exa == 0 ? colq >= 0 : prow >= 0);
+                ie1 = se1 ? (exa == 0 ? idx_x(a, colq, y, kk) : idx_y(a, x, prow, kk)) : 0;
+                const int k0 = 9 + exa;
+                ldg4_into(e1[0], a.mvi[k0] + ie1, se1); ldg4_into(e1[1], a.mvi[k0 + 3] + ie1, se1); ldg4_into(e1[2], a.mvi[k0 + 6] + ie1, se1);
+            }
+        }
         mbar_wait(&barG[it & 1], (it >> 1) & 1);
 
         const int s3 = it % 3, s3n = (it + 1) % 3;
@@ -546,14 +568,16 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                     const float4 o12 = ld4s(sm + FT_OFF_S12 + (it & 1) * FT_BOX, q);
                     if (exa == 0) {
                         const float4 o11 = ld4s(sm + FT_OFF_S11 + (it & 1) * FT_UPL, uq);
-                        X0 = adj_x_own(a, a.mvi[9], a.mvo[9], XT(T_A_INT), XT(T_B_INT), x, y, kk, colq, o11, wr);
-                        X1 = adj_x_own(a, a.mvi[12], a.mvo[12], XT(T_A_HALF), XT(T_B_HALF), x, y, kk, colq, o12, wr);
-                        X2 = adj_x_own(a, a.mvi[15], a.mvo[15], XT(T_A_HALF), XT(T_B_HALF), x, y, kk, colq, w13c, wr);
+                        const float4 ai = tab4(XT(T_A_INT), x), bi = tab4(XT(T_B_INT), x), ah = tab4(XT(T_A_HALF), x), bh = tab4(XT(T_B_HALF), x);
+                        X0 = adj_own_x(e1[0], a.mvo[9], ie1, se1, ai, bi, o11, wr);
+                        X1 = adj_own_x(e1[1], a.mvo[12], ie1, se1, ah, bh, o12, wr);
+                        X2 = adj_own_x(e1[2], a.mvo[15], ie1, se1, ah, bh, w13c, wr);
                     } else {
                         const float4 o22 = ld4s(sm + FT_OFF_S22 + (it & 1) * FT_BOX, q);
-                        X0 = adj_y_own(a, a.mvi[10], a.mvo[10], YT(T_A_HALF), YT(T_B_HALF), x, y, kk, prow, o12, wr);
-                        X1 = adj_y_own(a, a.mvi[13], a.mvo[13], YT(T_A_INT), YT(T_B_INT), x, y, kk, prow, o22, wr);
-                        X2 = adj_y_own(a, a.mvi[16], a.mvo[16], YT(T_A_HALF), YT(T_B_HALF), x, y, kk, prow, w23c, wr);
+                        const float4 ai = f4(YT(T_A_INT)[y]), bi = f4(YT(T_B_INT)[y]), ah = f4(YT(T_A_HALF)[y]), bh = f4(YT(T_B_HALF)[y]);
+                        X0 = adj_own_x(e1[0], a.mvo[10], ie1, se1, ah, bh, o12, wr);
+                        X1 = adj_own_x(e1[1], a.mvo[13], ie1, se1, ai, bi, o22, wr);
+                        X2 = adj_own_x(e1[2], a.mvo[16], ie1, se1, ah, bh, w23c, wr);
                     }
                 }
                 *reinterpret_cast<float4*>(SC1 + 0 * FT_RING * FT_UPL + 4 * uq) = X0;
@@ -707,6 +731,18 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                 ldg4_into(qm[2], a.mvi[11] + iz, ez); ldg4_into(qm[5], a.mvi[14] + iz, ez); ldg4_into(qm[8], a.mvi[17] + iz, ez);
             }
         }
+        // adjoint exchange CTAs: the three old T' of the own quad (plane ks = kk - 2) for the pre-block of stage 2
+        float4 e2[3];
+        bool se2 = false;
+        if (MODE == FM_ADJ) {
+            e2[0] = e2[1] = e2[2] = f4(0.0f);
+            if (exa >= 0 && it >= 4) {
+                const bool ok = pok && (unsigned)(kk - 2) < (unsigned)a.nz;
+                se2 = ok && (exa == 0 ? colq >= 0 : prow >= 0);
+                const long long i2 = se2 ? (exa == 0 ? idx_x(a, colq, y, kk - 2) : idx_y(a, x, prow, kk - 2)) : 0;
+                ldg4_into(e2[0], a.mvi[exa] + i2, se2); ldg4_into(e2[1], a.mvi[3 + exa] + i2, se2); ldg4_into(e2[2], a.mvi[6 + exa] + i2, se2);
+            }
+        }
         if (pml && tid >= 360 && tid < 364) {   // z table ring: plane kk + 3 (first read after the barrier)
             const int t = tid - 360, z = kk + 3;
             sm[FT_OFF_ZT + t * FT_ZRING + (z & (FT_ZRING - 1))] = (unsigned)z < (unsigned)a.nz ? __ldg(a.tab[2][t] + z) : 0.0f;
@@ -744,13 +780,15 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                     const float4 v2 = ld4s(sm + FT_OFF_UR + 1 * FT_RING * FT_UPL + pc, uq);
                     const float4 v3 = ld4s(sm + FT_OFF_UR + 2 * FT_RING * FT_UPL + pc, uq);
                     if (exa == 0) {
-                        Y0 = adj_x_own(a, a.mvi[0], nullptr, XT(T_A_HALF), XT(T_B_HALF), x, y, ks, colq, v1, false);
-                        Y1 = adj_x_own(a, a.mvi[3], nullptr, XT(T_A_INT), XT(T_B_INT), x, y, ks, colq, v2, false);
-                        Y2 = adj_x_own(a, a.mvi[6], nullptr, XT(T_A_INT), XT(T_B_INT), x, y, ks, colq, v3, false);
+                        const float4 ai = tab4(XT(T_A_INT), x), bi = tab4(XT(T_B_INT), x);
+                        Y0 = adj_own_x(e2[0], nullptr, 0, se2, tab4(XT(T_A_HALF), x), tab4(XT(T_B_HALF), x), v1, false);
+                        Y1 = adj_own_x(e2[1], nullptr, 0, se2, ai, bi, v2, false);
+                        Y2 = adj_own_x(e2[2], nullptr, 0, se2, ai, bi, v3, false);
                     } else {
-                        Y0 = adj_y_own(a, a.mvi[1], nullptr, YT(T_A_INT), YT(T_B_INT), x, y, ks, prow, v1, false);
-                        Y1 = adj_y_own(a, a.mvi[4], nullptr, YT(T_A_HALF), YT(T_B_HALF), x, y, ks, prow, v2, false);
-                        Y2 = adj_y_own(a, a.mvi[7], nullptr, YT(T_A_INT), YT(T_B_INT), x, y, ks, prow, v3, false);
+                        const float4 ai = f4(YT(T_A_INT)[y]), bi = f4(YT(T_B_INT)[y]);
+                        Y0 = adj_own_x(e2[0], nullptr, 0, se2, ai, bi, v1, false);
+                        Y1 = adj_own_x(e2[1], nullptr, 0, se2, f4(YT(T_A_HALF)[y]), f4(YT(T_B_HALF)[y]), v2, false);
+                        Y2 = adj_own_x(e2[2], nullptr, 0, se2, ai, bi, v3, false);
                     }
                 }
                 *reinterpret_cast<float4*>(SC2a + 4 * uq) = Y0;
