@@ -691,29 +691,6 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                 store_quad(a.out + U1 * box + g, n1, x, a.nx);
                 store_quad(a.out + U2 * box + g, n2, x, a.nx);
                 store_quad(a.out + U3 * box + g, n3, x, a.nx);
-                if (MODE == FM_ADJ && pml1) {   // phi_bar (tilde form) fed by the new u_bar: Eq. 61c,e in scaled variables
-                    if (colq >= 0) {
-                        const long long i = idx_x(a, colq, y, kk);
-                        const float4 bi = tab4(XT(T_B_INT), x);
-                        adj_own(a.mvi[0], a.mvo[0], i, tab4(XT(T_B_HALF), x), n1);
-                        adj_own(a.mvi[3], a.mvo[3], i, bi, n2);
-                        adj_own(a.mvi[6], a.mvo[6], i, bi, n3);
-                    }
-                    if (prow >= 0) {
-                        const long long i = idx_y(a, x, prow, kk);
-                        const float bi = YT(T_B_INT)[y];
-                        adj_own(a.mvi[1], a.mvo[1], i, bi, n1);
-                        adj_own(a.mvi[4], a.mvo[4], i, YT(T_B_HALF)[y], n2);
-                        adj_own(a.mvi[7], a.mvo[7], i, bi, n3);
-                    }
-                    if (pz >= 0) {
-                        const long long i = idx_z(a, x, y, pz);
-                        const float bi = ZT(T_B_INT)[kk & (FT_ZRING - 1)];
-                        adj_own(a.mvi[2], a.mvo[2], i, bi, n1);
-                        adj_own(a.mvi[5], a.mvo[5], i, bi, n2);
-                        adj_own(a.mvi[8], a.mvo[8], i, ZT(T_B_HALF)[kk & (FT_ZRING - 1)], n3);
-                    }
-                }
             }
         }
         // forward C-PML: the nine psi of the quad at plane ks = kk - 2, issued ahead of the barrier
@@ -733,13 +710,14 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
         }
         // adjoint exchange CTAs: the three old T' of the own quad (plane ks = kk - 2) for the pre-block of stage 2
         float4 e2[3];
+        long long i2 = 0;
         bool se2 = false;
         if (MODE == FM_ADJ) {
             e2[0] = e2[1] = e2[2] = f4(0.0f);
             if (exa >= 0 && it >= 4) {
                 const bool ok = pok && (unsigned)(kk - 2) < (unsigned)a.nz;
                 se2 = ok && (exa == 0 ? colq >= 0 : prow >= 0);
-                const long long i2 = se2 ? (exa == 0 ? idx_x(a, colq, y, kk - 2) : idx_y(a, x, prow, kk - 2)) : 0;
+                i2 = se2 ? (exa == 0 ? idx_x(a, colq, y, kk - 2) : idx_y(a, x, prow, kk - 2)) : 0;
                 ldg4_into(e2[0], a.mvi[exa] + i2, se2); ldg4_into(e2[1], a.mvi[3 + exa] + i2, se2); ldg4_into(e2[2], a.mvi[6 + exa] + i2, se2);
             }
         }
@@ -781,14 +759,14 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                     const float4 v3 = ld4s(sm + FT_OFF_UR + 2 * FT_RING * FT_UPL + pc, uq);
                     if (exa == 0) {
                         const float4 ai = tab4(XT(T_A_INT), x), bi = tab4(XT(T_B_INT), x);
-                        Y0 = adj_own_x(e2[0], nullptr, 0, se2, tab4(XT(T_A_HALF), x), tab4(XT(T_B_HALF), x), v1, false);
-                        Y1 = adj_own_x(e2[1], nullptr, 0, se2, ai, bi, v2, false);
-                        Y2 = adj_own_x(e2[2], nullptr, 0, se2, ai, bi, v3, false);
+                        Y0 = adj_own_x(e2[0], a.mvo[0], i2, se2, tab4(XT(T_A_HALF), x), tab4(XT(T_B_HALF), x), v1, inner);
+                        Y1 = adj_own_x(e2[1], a.mvo[3], i2, se2, ai, bi, v2, inner);
+                        Y2 = adj_own_x(e2[2], a.mvo[6], i2, se2, ai, bi, v3, inner);
                     } else {
                         const float4 ai = f4(YT(T_A_INT)[y]), bi = f4(YT(T_B_INT)[y]);
-                        Y0 = adj_own_x(e2[0], nullptr, 0, se2, ai, bi, v1, false);
-                        Y1 = adj_own_x(e2[1], nullptr, 0, se2, f4(YT(T_A_HALF)[y]), f4(YT(T_B_HALF)[y]), v2, false);
-                        Y2 = adj_own_x(e2[2], nullptr, 0, se2, ai, bi, v3, false);
+                        Y0 = adj_own_x(e2[0], a.mvo[1], i2, se2, ai, bi, v1, inner);
+                        Y1 = adj_own_x(e2[1], a.mvo[4], i2, se2, f4(YT(T_A_HALF)[y]), f4(YT(T_B_HALF)[y]), v2, inner);
+                        Y2 = adj_own_x(e2[2], a.mvo[7], i2, se2, ai, bi, v3, inner);
                     }
                 }
                 *reinterpret_cast<float4*>(SC2a + 4 * uq) = Y0;
@@ -826,10 +804,10 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                 }
                 if (MODE == FM_ADJ && pml2) {
                     if (exa == 0) e11 = e11 + dmx(ld2s(SC2a, 4 * uq - 2), ld4s(SC2a, uq), ld2s(SC2a, 4 * uq + 4));
-                    else if (nearx) { const Taps8 X = adj_x(a, a.mvi[0], nullptr, XT(T_A_HALF), XT(T_B_HALF), x, y, ks, l, c, rr, false); e11 = e11 + dmx(X.l, X.c, X.r); }
+                    else if (nearx) { const Taps8 X = adj_x(a, a.mvi[0], a.mvo[0], XT(T_A_HALF), XT(T_B_HALF), x, y, ks, l, c, rr, true); e11 = e11 + dmx(X.l, X.c, X.r); }
                     if (exa == 1) g12 = g12 + d4(ld4s(SC2a, uq - 10), ld4s(SC2a, uq), ld4s(SC2a, uq + 10), ld4s(SC2a, uq + 20));
-                    else if (neary) g12 = g12 + adj_y(a, a.mvi[1], nullptr, YT(T_A_INT), YT(T_B_INT), x, y - 1, ks, 1, ya, c, yc, yd, false);
-                    if (bz) g13 = g13 + adj_z(a, a.mvi[2], nullptr, ZT(T_A_INT), ZT(T_B_INT), x, y, ks - 1, 1, za, c, zc, zd, false);
+                    else if (neary) g12 = g12 + adj_y(a, a.mvi[1], a.mvo[1], YT(T_A_INT), YT(T_B_INT), x, y - 1, ks, 1, ya, c, yc, yd, true);
+                    if (bz) g13 = g13 + adj_z(a, a.mvi[2], a.mvo[2], ZT(T_A_INT), ZT(T_B_INT), x, y, ks - 1, 1, za, c, zc, zd, true);
                 }
             }
             {   // ---- derivatives of u2: D+x (g21), D-y (e22), D+z (g23)
@@ -845,10 +823,10 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                 }
                 if (MODE == FM_ADJ && pml2) {
                     if (exa == 0) g21 = g21 + dpx(ld2s(SC2b, 4 * uq - 2), ld4s(SC2b, uq), ld2s(SC2b, 4 * uq + 4));
-                    else if (nearx) { const Taps8 X = adj_x(a, a.mvi[3], nullptr, XT(T_A_INT), XT(T_B_INT), x, y, ks, l, c, rr, false); g21 = g21 + dpx(X.l, X.c, X.r); }
+                    else if (nearx) { const Taps8 X = adj_x(a, a.mvi[3], a.mvo[3], XT(T_A_INT), XT(T_B_INT), x, y, ks, l, c, rr, true); g21 = g21 + dpx(X.l, X.c, X.r); }
                     if (exa == 1) e22 = e22 + d4(ld4s(SC2b, uq - 20), ld4s(SC2b, uq - 10), ld4s(SC2b, uq), ld4s(SC2b, uq + 10));
-                    else if (neary) e22 = e22 + adj_y(a, a.mvi[4], nullptr, YT(T_A_HALF), YT(T_B_HALF), x, y - 2, ks, 2, ya, yb, c, yd, false);
-                    if (bz) g23 = g23 + adj_z(a, a.mvi[5], nullptr, ZT(T_A_INT), ZT(T_B_INT), x, y, ks - 1, 1, za, c, zc, zd, false);
+                    else if (neary) e22 = e22 + adj_y(a, a.mvi[4], a.mvo[4], YT(T_A_HALF), YT(T_B_HALF), x, y - 2, ks, 2, ya, yb, c, yd, true);
+                    if (bz) g23 = g23 + adj_z(a, a.mvi[5], a.mvo[5], ZT(T_A_INT), ZT(T_B_INT), x, y, ks - 1, 1, za, c, zc, zd, true);
                 }
             }
             {   // ---- derivatives of u3: D+x (g31), D+y (g32), D-z (e33)
@@ -864,10 +842,10 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                 }
                 if (MODE == FM_ADJ && pml2) {
                     if (exa == 0) g31 = g31 + dpx(ld2s(SC2c, 4 * uq - 2), ld4s(SC2c, uq), ld2s(SC2c, 4 * uq + 4));
-                    else if (nearx) { const Taps8 X = adj_x(a, a.mvi[6], nullptr, XT(T_A_INT), XT(T_B_INT), x, y, ks, l, c, rr, false); g31 = g31 + dpx(X.l, X.c, X.r); }
+                    else if (nearx) { const Taps8 X = adj_x(a, a.mvi[6], a.mvo[6], XT(T_A_INT), XT(T_B_INT), x, y, ks, l, c, rr, true); g31 = g31 + dpx(X.l, X.c, X.r); }
                     if (exa == 1) g32 = g32 + d4(ld4s(SC2c, uq - 10), ld4s(SC2c, uq), ld4s(SC2c, uq + 10), ld4s(SC2c, uq + 20));
-                    else if (neary) g32 = g32 + adj_y(a, a.mvi[7], nullptr, YT(T_A_INT), YT(T_B_INT), x, y - 1, ks, 1, ya, c, yc, yd, false);
-                    if (bz) e33 = e33 + adj_z(a, a.mvi[8], nullptr, ZT(T_A_HALF), ZT(T_B_HALF), x, y, ks - 2, 2, za, zb_, c, zd, false);
+                    else if (neary) g32 = g32 + adj_y(a, a.mvi[7], a.mvo[7], YT(T_A_INT), YT(T_B_INT), x, y - 1, ks, 1, ya, c, yc, yd, true);
+                    if (bz) e33 = e33 + adj_z(a, a.mvi[8], a.mvo[8], ZT(T_A_HALF), ZT(T_B_HALF), x, y, ks - 2, 2, za, zb_, c, zd, true);
                 }
             }
 
