@@ -291,22 +291,30 @@ __device__ __forceinline__ Taps8 adj_x(const FusedArgs& a, const float* __restri
     return X;
 }
 // X along y: rows r0..r0+3 of plane z at the thread's quad ; tap `own` is the thread's own row.  Returns d4 of X.
+// The four loads are predicated, not branched around, so that they issue back to back.
 __device__ __forceinline__ float4 adj_y(const FusedArgs& a, const float* __restrict__ Ti, float* __restrict__ To,
                                         const float* __restrict__ ta, const float* __restrict__ tb,
                                         int x, int r0, int z, int own, float4 s0, float4 s1, float4 s2, float4 s3, bool wr)
 {
     const float4 s[4] = {s0, s1, s2, s3};
+    float4 T[4];
+    long long i[4];
+    bool in[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int p = yzslab_row(r0 + k, a.ny, a.P);
+        in[k] = p >= 0;
+        i[k] = in[k] ? idx_y(a, x, p, z) : 0;
+        T[k] = f4(0.0f);
+        ldg4_into(T[k], Ti + i[k], in[k]);
+    }
     float4 X[4];
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-        X[k] = f4(0.0f);
-        const int p = yzslab_row(r0 + k, a.ny, a.P);
-        if (p >= 0) {
-            const long long i = idx_y(a, x, p, z);
-            const float4 Tn = fma4(tb[r0 + k], ldg4(Ti + i), s[k]);
-            if (wr && k == own) stg4(To + i, Tn);
-            X[k] = ta[r0 + k] * Tn;
-        }
+        const float bk = in[k] ? tb[r0 + k] : 0.0f, ak = in[k] ? ta[r0 + k] : 0.0f;
+        const float4 Tn = fma4(bk, T[k], s[k]);
+        if (wr && k == own && in[k]) stg4(To + i[k], Tn);
+        X[k] = ak * Tn;
     }
     return d4(X[0], X[1], X[2], X[3]);
 }
@@ -316,17 +324,24 @@ __device__ __forceinline__ float4 adj_z(const FusedArgs& a, const float* __restr
                                         int x, int y, int z0, int own, float4 s0, float4 s1, float4 s2, float4 s3, bool wr)
 {
     const float4 s[4] = {s0, s1, s2, s3};
+    float4 T[4];
+    long long i[4];
+    bool in[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int p = yzslab_row(z0 + k, a.nz, a.P);
+        in[k] = p >= 0;
+        i[k] = in[k] ? idx_z(a, x, y, p) : 0;
+        T[k] = f4(0.0f);
+        ldg4_into(T[k], Ti + i[k], in[k]);
+    }
     float4 X[4];
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-        X[k] = f4(0.0f);
-        const int p = yzslab_row(z0 + k, a.nz, a.P);
-        if (p >= 0) {
-            const long long i = idx_z(a, x, y, p);
-            const float4 Tn = fma4(tb[(z0 + k) & (FT_ZRING - 1)], ldg4(Ti + i), s[k]);
-            if (wr && k == own) stg4(To + i, Tn);
-            X[k] = ta[(z0 + k) & (FT_ZRING - 1)] * Tn;
-        }
+        const float bk = tb[(z0 + k) & (FT_ZRING - 1)], ak = in[k] ? ta[(z0 + k) & (FT_ZRING - 1)] : 0.0f;
+        const float4 Tn = fma4(bk, T[k], s[k]);
+        if (wr && k == own && in[k]) stg4(To + i[k], Tn);
+        X[k] = ak * Tn;
     }
     return d4(X[0], X[1], X[2], X[3]);
 }
