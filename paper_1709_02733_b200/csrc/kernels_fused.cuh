@@ -124,13 +124,6 @@ __device__ __forceinline__ void tma_plane(const CUtensorMap* tm, float* dst, uin
         : "memory");
 }
 
-// the same box, only pulled into L2 (no shared-memory destination, no barrier)
-__device__ __forceinline__ void tma_prefetch_plane(const CUtensorMap* tm, int c0, int c1, int c2, int c3)
-{
-    asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];"
-                 ::"l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
-}
-
 // ---- float4 helpers -----------------------------------------------------------------------------
 __device__ __forceinline__ float4 ld4s(const float* p, int quad) { return *reinterpret_cast<const float4*>(p + 4 * quad); }
 __device__ __forceinline__ float2 ld2s(const float* p, int off) { return *reinterpret_cast<const float2*>(p + off); }
@@ -260,36 +253,6 @@ __device__ __forceinline__ float4 pml_fwd_m(float4 m_old, float* mo, long long i
 // Transposed recursion in tilde form (Eq. 61b / 61d-g): T <- b T + s at the
 // sample, and the differenced quantity is s + a T.  The a T part ("X") is needed at every tap of
 // the difference along the slab axis, so it is re-derived from the neighbours' old T.
-struct Taps8 { float2 l; float4 c; float2 r; };   // x-2,x-1 | x..x+3 | x+4,x+5
-
-// X along x for the row (y,z) of memory variable (Ti -> To); s = (l, c, r) are the samples at x-2..x+5
-__device__ __forceinline__ Taps8 adj_x(const FusedArgs& a, const float* __restrict__ Ti, float* __restrict__ To,
-                                       const float* __restrict__ ta, const float* __restrict__ tb,
-                                       int x, int y, int z, float2 l, float4 c, float2 r, bool wr)
-{
-    Taps8 X;
-    X.l = make_float2(0.0f, 0.0f); X.c = f4(0.0f); X.r = make_float2(0.0f, 0.0f);
-    const long long row = idx_x(a, 0, y, z);
-    int col = xslab_col(a, x);
-    if (col >= 0) {
-        const float4 Tn = fma4(tab4(tb, x), ldg4(Ti + row + col), c);
-        if (wr) stg4(To + row + col, Tn);
-        X.c = tab4(ta, x) * Tn;
-    }
-    col = xslab_col(a, x - 4);
-    if (col >= 0) {
-        const float4 T = ldg4(Ti + row + col);
-        X.l.x = ta[x - 2] * fmaf(tb[x - 2], T.z, l.x);
-        X.l.y = ta[x - 1] * fmaf(tb[x - 1], T.w, l.y);
-    }
-    col = xslab_col(a, x + 4);
-    if (col >= 0) {
-        const float4 T = ldg4(Ti + row + col);
-        X.r.x = ta[x + 4] * fmaf(tb[x + 4], T.x, r.x);
-        X.r.y = ta[x + 5] * fmaf(tb[x + 5], T.y, r.y);
-    }
-    return X;
-}
 // X along y: rows r0..r0+3 of plane z at the thread's quad ; tap `own` is the thread's own row.  Returns d4 of X.
 // The four loads are predicated, not branched around, so that they issue back to back.
 __device__ __forceinline__ float4 adj_y(const FusedArgs& a, const float* __restrict__ Ti, float* __restrict__ To,
@@ -345,26 +308,6 @@ __device__ __forceinline__ float4 adj_z(const FusedArgs& a, const float* __restr
     }
     return d4(X[0], X[1], X[2], X[3]);
 }
-// Own-quad part of the same: T <- b T + s (stored by the owner) ; returns X = a T, zero outside the slab.  Used when
-// the CTA exchanges X through shared memory instead of re-deriving the neighbours' values (one slab axis per CTA).
-__device__ __forceinline__ float4 adj_x_own(const FusedArgs& a, const float* __restrict__ Ti, float* __restrict__ To,
-                                            const float* ta, const float* tb, int x, int y, int z, int col, float4 s, bool wr)
-{
-    if (col < 0) return f4(0.0f);
-    const long long i = idx_x(a, col, y, z);
-    const float4 Tn = fma4(tab4(tb, x), ldg4(Ti + i), s);
-    if (wr) stg4(To + i, Tn);
-    return tab4(ta, x) * Tn;
-}
-__device__ __forceinline__ float4 adj_y_own(const FusedArgs& a, const float* __restrict__ Ti, float* __restrict__ To,
-                                            const float* ta, const float* tb, int x, int y, int z, int row, float4 s, bool wr)
-{
-    if (row < 0) return f4(0.0f);
-    const long long i = idx_y(a, x, row, z);
-    const float4 Tn = fma4(tb[y], ldg4(Ti + i), s);
-    if (wr) stg4(To + i, Tn);
-    return ta[y] * Tn;
-}
 // the same with the old T already in registers (loaded ahead of a barrier)
 __device__ __forceinline__ float4 adj_own_x(float4 Told, float* To, long long i, bool in_slab, float4 a4, float4 b4, float4 s, bool wr)
 {
@@ -373,10 +316,6 @@ __device__ __forceinline__ float4 adj_own_x(float4 Told, float* To, long long i,
     if (wr) stg4(To + i, Tn);
     return a4 * Tn;
 }
-// tilde-form update of an own-quad memory variable fed by the new value v: T <- b T + v
-__device__ __forceinline__ void adj_own(const float* Ti, float* To, long long i, float4 b4, float4 v) { stg4(To + i, fma4(b4, ldg4(Ti + i), v)); }
-__device__ __forceinline__ void adj_own(const float* Ti, float* To, long long i, float b1, float4 v) { stg4(To + i, fma4(b1, ldg4(Ti + i), v)); }
-
 // =================================================================================================
 // The fused step.  MODE selects the C-PML code carried by the launch (FM_*); see DESIGN.md for the
 // index algebra.  Relative plane j <-> z = zb - 2 + j ; iteration `it` computes u(kk = zb - 2 + it)
@@ -424,8 +363,8 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
     const bool pok = pml && act1 && x >= 0 && x < a.nxq && yin;     // quad has memory-variable storage (given z in range)
     const int colq = pok ? xslab_col(a, x) : -1;
     const int prow = pok ? yzslab_row(y, a.ny, a.P) : -1;
-    // adjoint: does any tap of this thread's differences along x / y fall into a slab
-    const bool nearx = pok && (colq >= 0 || xslab_col(a, x - 4) >= 0 || xslab_col(a, x + 4) >= 0);
+    // adjoint: does any tap of this thread's differences along y fall into a slab (x taps always go through the
+    // shared-memory exchange: a CTA that touches the x slabs takes x as its exchange axis)
     const bool neary = pok && (y - 2 < a.P || y + 2 >= a.ny - 1 - a.P);
 
     // adjoint: slab axis whose filtered taps this CTA exchanges through shared memory (x if it touches the x slabs,
@@ -643,7 +582,6 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                 if (MODE == FM_ADJ && pml1) {
                     const float* S = SC1 + 0 * FT_RING * FT_UPL;
                     if (exa == 0) t1 = t1 + dpx(ld2s(S, 4 * uq - 2), ld4s(S, uq), ld2s(S, 4 * uq + 4));
-                    else if (nearx) { const Taps8 X = adj_x(a, a.mvi[9], a.mvo[9], XT(T_A_INT), XT(T_B_INT), x, y, kk, l, c11, rr, wr1); t1 = t1 + dpx(X.l, X.c, X.r); }
                     if (yex) t2 = t2 + d4(ld4s(S, uq - 20), ld4s(S, uq - 10), ld4s(S, uq), ld4s(S, uq + 10));
                     else if (neary) t2 = t2 + adj_y(a, a.mvi[10], a.mvo[10], YT(T_A_HALF), YT(T_B_HALF), x, y - 2, kk, 2, ya, yb, c12, yd, wr1 && exa != 1);
                     if (bz) t3 = t3 + adj_z(a, a.mvi[11], a.mvo[11], ZT(T_A_HALF), ZT(T_B_HALF), x, y, kk - 2, 2, w13a, w13b, w13c, f13, wr1);
@@ -664,7 +602,6 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                 if (MODE == FM_ADJ && pml1) {
                     const float* S = SC1 + 1 * FT_RING * FT_UPL;
                     if (exa == 0) t1 = t1 + dmx(ld2s(S, 4 * uq - 2), ld4s(S, uq), ld2s(S, 4 * uq + 4));
-                    else if (nearx) { const Taps8 X = adj_x(a, a.mvi[12], a.mvo[12], XT(T_A_HALF), XT(T_B_HALF), x, y, kk, l, c12, rr, wr1); t1 = t1 + dmx(X.l, X.c, X.r); }
                     if (yex) t2 = t2 + d4(ld4s(S, uq - 10), ld4s(S, uq), ld4s(S, uq + 10), ld4s(S, uq + 20));
                     else if (neary) t2 = t2 + adj_y(a, a.mvi[13], a.mvo[13], YT(T_A_INT), YT(T_B_INT), x, y - 1, kk, 1, yb, c22, yc, yd, wr1 && exa != 1);
                     if (bz) t3 = t3 + adj_z(a, a.mvi[14], a.mvo[14], ZT(T_A_HALF), ZT(T_B_HALF), x, y, kk - 2, 2, w23a, w23b, w23c, f23, wr1);
@@ -684,7 +621,6 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                 if (MODE == FM_ADJ && pml1) {
                     const float* S = SC1 + 2 * FT_RING * FT_UPL;
                     if (exa == 0) t1 = t1 + dmx(ld2s(S, 4 * uq - 2), ld4s(S, uq), ld2s(S, 4 * uq + 4));
-                    else if (nearx) { const Taps8 X = adj_x(a, a.mvi[15], a.mvo[15], XT(T_A_HALF), XT(T_B_HALF), x, y, kk, l, w13c, rr, wr1); t1 = t1 + dmx(X.l, X.c, X.r); }
                     if (yex) t2 = t2 + d4(ld4s(S, uq - 20), ld4s(S, uq - 10), ld4s(S, uq), ld4s(S, uq + 10));
                     else if (neary) t2 = t2 + adj_y(a, a.mvi[16], a.mvo[16], YT(T_A_HALF), YT(T_B_HALF), x, y - 2, kk, 2, ya, yb, w23c, yd, wr1 && exa != 1);
                     if (bz) t3 = t3 + adj_z(a, a.mvi[17], a.mvo[17], ZT(T_A_INT), ZT(T_B_INT), x, y, kk - 1, 1, w33b, w33c, w33d, f33, wr1);
@@ -819,7 +755,6 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                 }
                 if (MODE == FM_ADJ && pml2) {
                     if (exa == 0) e11 = e11 + dmx(ld2s(SC2a, 4 * uq - 2), ld4s(SC2a, uq), ld2s(SC2a, 4 * uq + 4));
-                    else if (nearx) { const Taps8 X = adj_x(a, a.mvi[0], a.mvo[0], XT(T_A_HALF), XT(T_B_HALF), x, y, ks, l, c, rr, true); e11 = e11 + dmx(X.l, X.c, X.r); }
                     if (exa == 1) g12 = g12 + d4(ld4s(SC2a, uq - 10), ld4s(SC2a, uq), ld4s(SC2a, uq + 10), ld4s(SC2a, uq + 20));
                     else if (neary) g12 = g12 + adj_y(a, a.mvi[1], a.mvo[1], YT(T_A_INT), YT(T_B_INT), x, y - 1, ks, 1, ya, c, yc, yd, true);
                     if (bz) g13 = g13 + adj_z(a, a.mvi[2], a.mvo[2], ZT(T_A_INT), ZT(T_B_INT), x, y, ks - 1, 1, za, c, zc, zd, true);
@@ -838,7 +773,6 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                 }
                 if (MODE == FM_ADJ && pml2) {
                     if (exa == 0) g21 = g21 + dpx(ld2s(SC2b, 4 * uq - 2), ld4s(SC2b, uq), ld2s(SC2b, 4 * uq + 4));
-                    else if (nearx) { const Taps8 X = adj_x(a, a.mvi[3], a.mvo[3], XT(T_A_INT), XT(T_B_INT), x, y, ks, l, c, rr, true); g21 = g21 + dpx(X.l, X.c, X.r); }
                     if (exa == 1) e22 = e22 + d4(ld4s(SC2b, uq - 20), ld4s(SC2b, uq - 10), ld4s(SC2b, uq), ld4s(SC2b, uq + 10));
                     else if (neary) e22 = e22 + adj_y(a, a.mvi[4], a.mvo[4], YT(T_A_HALF), YT(T_B_HALF), x, y - 2, ks, 2, ya, yb, c, yd, true);
                     if (bz) g23 = g23 + adj_z(a, a.mvi[5], a.mvo[5], ZT(T_A_INT), ZT(T_B_INT), x, y, ks - 1, 1, za, c, zc, zd, true);
@@ -857,7 +791,6 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                 }
                 if (MODE == FM_ADJ && pml2) {
                     if (exa == 0) g31 = g31 + dpx(ld2s(SC2c, 4 * uq - 2), ld4s(SC2c, uq), ld2s(SC2c, 4 * uq + 4));
-                    else if (nearx) { const Taps8 X = adj_x(a, a.mvi[6], a.mvo[6], XT(T_A_INT), XT(T_B_INT), x, y, ks, l, c, rr, true); g31 = g31 + dpx(X.l, X.c, X.r); }
                     if (exa == 1) g32 = g32 + d4(ld4s(SC2c, uq - 10), ld4s(SC2c, uq), ld4s(SC2c, uq + 10), ld4s(SC2c, uq + 20));
                     else if (neary) g32 = g32 + adj_y(a, a.mvi[7], a.mvo[7], YT(T_A_INT), YT(T_B_INT), x, y - 1, ks, 1, ya, c, yc, yd, true);
                     if (bz) e33 = e33 + adj_z(a, a.mvi[8], a.mvo[8], ZT(T_A_HALF), ZT(T_B_HALF), x, y, ks - 2, 2, za, zb_, c, zd, true);

@@ -174,6 +174,23 @@ def test_config4_full_size_truncated(torch_cuda):
     assert abs(a - b) <= TOL_DOT * max(abs(a), abs(b))
 
 
+def test_fused_is_bitwise_repeatable(torch_cuda):
+    """The fused kernel synchronises with one block barrier per plane plus mbarriers, re-uses shared-memory slots
+    as soon as their last reader has passed a barrier, and runs interior and slab bricks on two streams: a missed
+    hazard would show up as run-to-run differences.  Five runs of H and H^T on a 3 x 3 tile grid with several z
+    chunks (x, y and z slabs, corner tiles) must agree bit for bit.  (compute-sanitizer is closed on this pool.)"""
+    torch = torch_cuda
+    prob = synth.random_problem(nx=90, ny=75, nz=50, nt=14, npml=7, L=17, seed=31, lossy=True)
+    x, y = synth.random_vectors(prob, seed=31)
+    ctx = gpu_ops(torch, prob, variant=2, graph=0, zchunk=9)
+    xd, yd = torch.from_numpy(x.astype(np.float32)).cuda(), torch.from_numpy(y.astype(np.float32)).cuda()
+    d0, i0 = ctx.forward(xd).clone(), ctx.adjoint(yd).clone()
+    for _ in range(4):
+        assert torch.equal(ctx.forward(xd), d0)
+        assert torch.equal(ctx.adjoint(yd), i0)
+    ctx.close()
+
+
 def test_graph_and_direct_launch_agree_bitwise(torch_cuda):
     prob = synth.random_problem(nx=40, ny=24, nz=33, nt=30, npml=4, L=7, seed=6)
     x, y = synth.random_vectors(prob, seed=6)
