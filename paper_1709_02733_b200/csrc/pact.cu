@@ -511,7 +511,7 @@ static int ensure_fused(pact_ctx* c)
     CK(cudaFuncSetAttribute(k_fused<FM_ADJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
     fa.mat = g.Ll;
     c->work_zc = -1;
-    c->work_cap = (long long)((g.nx + FT_TX - 1) / FT_TX) * ((g.ny + FT_TY - 1) / FT_TY) * (g.nz + 2);
+    c->work_cap = (long long)((g.nx + FT_TX - 1) / FT_TX) * ((g.ny + FT_TY - 1) / FT_TY) * (2 * g.nz + 2);   // worst case: one-plane chunks
     for (int k = 0; k < 2; ++k)
         if ((rc = dev_alloc(c, (void**)&c->d_work[k], (size_t)c->work_cap * sizeof(int4)))) return rc;
     CK(cudaStreamCreateWithFlags(&c->aux_stream, cudaStreamNonBlocking));

@@ -64,6 +64,7 @@ RANDOM_CASES = [
     dict(nx=70, ny=34, nz=29, nt=30, npml=4, L=11, seed=2, lossy=True),
     dict(nx=33, ny=66, nz=20, nt=25, npml=0, L=9, seed=3, lossy=False),
     dict(nx=75, ny=70, nz=23, nt=22, npml=6, L=13, seed=21, lossy=True),     # 3 x 3 fused tiles, ragged
+    dict(nx=100, ny=90, nz=84, nt=16, npml=36, L=9, seed=25, lossy=True),    # C-PML thicker than a tile: whole tiles inside slabs
     dict(nx=8, ny=8, nz=8, nt=12, npml=0, L=3, seed=4, lossy=True),          # minimum grid
     dict(nx=16, ny=17, nz=18, nt=20, npml=4, L=5, seed=5, lossy=True),       # 2*npml+8 == nx: thickest legal PML
 ]
@@ -97,6 +98,20 @@ def test_config1_full(torch_cuda, variant):
     assert rel_l2(Hty, Hty_o) <= TOL_L2
     y32 = y.astype(np.float32).astype(np.float64)
     a, b = np.vdot(Hx.astype(np.float64), y32), np.vdot(prob.p0.astype(np.float64), Hty.astype(np.float64))
+    assert abs(a - b) <= TOL_DOT * max(abs(a), abs(b))
+
+
+def test_config3_truncated(torch_cuda):
+    """BASELINE config 3 (256^3 porous skull, hemispherical array) on its real volumes, 24 samples, automatic
+    variant (fused), random x and y: parity and dot test."""
+    prob = synth.make_config(3, nt=24)
+    x, y = synth.random_vectors(prob, seed=43)
+    Hx, Hty = run_pair(torch_cuda, prob, x, y, variant=0)
+    Hx_o, Hty_o = oracle_pair(prob, x, y)
+    assert rel_l2(Hx, Hx_o) <= TOL_L2
+    assert rel_l2(Hty, Hty_o) <= TOL_L2
+    x32, y32 = x.astype(np.float32).astype(np.float64), y.astype(np.float32).astype(np.float64)
+    a, b = np.vdot(Hx.astype(np.float64), y32), np.vdot(x32, Hty.astype(np.float64))
     assert abs(a - b) <= TOL_DOT * max(abs(a), abs(b))
 
 
