@@ -588,32 +588,32 @@ static void fused_step(pact_ctx* c, Launcher& ln, int cur, float sgn, int kind)
     cudaStream_t st = c->stream, aux = c->aux_stream;
     const bool both = c->nwork[0] > 0 && c->nwork[1] > 0;
     if (both) { cudaEventRecord(c->ev_fork, st); cudaStreamWaitEvent(aux, c->ev_fork, 0); }
-    if (c->nwork[1] > 0) {      // the slab CTAs (slower per plane) start first
-        FusedArgs fb = fa;
-        fb.work = c->d_work[1];
-        cudaStream_t s1 = both ? aux : st;
+    FusedArgs fs = fa, fi = fa;
+    fs.work = c->d_work[1];
+    fi.work = c->d_work[0];
+    cudaStream_t s1 = both ? aux : st;
+    auto launch_slab = [&] {
         const int grid = c->nwork[1];
-        auto launch = [&] {
-            if (fa.P == 0) k_fused<FM_PLAIN><<<grid, FT_NT, FT_SMEM_BYTES, s1>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fb);
-            else if (sgn > 0.0f) k_fused<FM_FWD><<<grid, FT_NT, FT_SMEM_BYTES, s1>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fb);
-            else k_fused<FM_ADJ><<<grid, FT_NT, FT_SMEM_BYTES, s1>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fb);
-        };
-        if (both) {   // timed together with the interior launch below (they overlap); counted under PACT_K_OTHER
-            launch();
-            cudaEventRecord(c->ev_join, aux);
-            c->launches[ln.op][PACT_K_OTHER]++;
-        }
-        else ln.run(kind, launch);
+        if (fa.P == 0) k_fused<FM_PLAIN><<<grid, FT_NT, FT_SMEM_BYTES, s1>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fs);
+        else if (sgn > 0.0f) k_fused<FM_FWD><<<grid, FT_NT, FT_SMEM_BYTES, s1>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fs);
+        else k_fused<FM_ADJ><<<grid, FT_NT, FT_SMEM_BYTES, s1>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fs);
+    };
+    auto launch_int = [&] {
+        k_fused<FM_PLAIN><<<c->nwork[0], FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fi);
+    };
+    if (!both) {
+        if (c->nwork[1] > 0) ln.run(kind, launch_slab);
+        if (c->nwork[0] > 0) ln.run(kind, launch_int);
+        return;
     }
-    if (c->nwork[0] > 0) {
-        FusedArgs fb = fa;
-        fb.work = c->d_work[0];
-        const int grid = c->nwork[0];
-        ln.run(kind, [&] {
-            k_fused<FM_PLAIN><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fb);
-            if (both) cudaStreamWaitEvent(st, c->ev_join, 0);
-        });
-    }
+    // both: timed as one (they overlap); the slab launch is counted under PACT_K_OTHER
+    ln.run(kind, [&] {
+        launch_slab();
+        launch_int();
+        cudaEventRecord(c->ev_join, aux);
+        cudaStreamWaitEvent(st, c->ev_join, 0);
+    });
+    c->launches[ln.op][PACT_K_OTHER]++;
 }
 
 // Eq. 58 right to left: tau, then for m = 0..M-1 { Theta ; W' unless m = M-1 }
