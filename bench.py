@@ -276,7 +276,7 @@ def main():
                 "adjoint_frac": B_ALG * prm.N / (t_adj * 1e-3) / 1e9 / peak,
                 "forward_loop_ms": loop_f, "adjoint_loop_ms": loop_a,
                 "kernel_ms": {"forward": {k: v for k, v in k_f.items() if v}, "adjoint": {k: v for k, v in k_a.items() if v}}}
-        tr = os.path.join(ROOT, "profiles", "traffic.json")   # per-launch DRAM bytes from the committed ncu capture
+        tr = os.path.join(ROOT, "profiles", "r1_traffic.txt")   # per-launch DRAM bytes from the committed ncu capture
         if os.path.exists(tr):
             try:
                 t = json.load(open(tr)).get(f"config{args.config}")
