@@ -187,6 +187,37 @@ def whole_job_rate(cells_per_rank_step, steps, world, ms_max):
     return world * cells_per_rank_step * steps / (ms_max * 1e-3) / 1e9
 
 
+def csrc_digest():
+    """sha256 over the CUDA sources: a committed ncu capture is only quoted while the kernels it measured
+    are the kernels that run."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_1709_02733_b200", "csrc")
+    for name in sorted(os.listdir(d)):
+        if name.endswith((".cu", ".cuh")):
+            h.update(open(os.path.join(d, name), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def committed_traffic(config):
+    """DRAM bytes per launch from the committed `ncu --set full` capture (profiles/traffic.txt), or (None, why).
+    Not measured in this run: the JSON line says so in `traffic_source`."""
+    path = os.path.join(ROOT, "profiles", "traffic.txt")
+    if not os.path.exists(path):
+        return None, "no committed capture (profiles/traffic.txt)"
+    try:
+        rec = json.load(open(path))
+        t = rec.get(f"config{config}")
+        if not t:
+            return None, f"profiles/traffic.txt has no capture of config {config}"
+        if rec.get("csrc_sha256_16") != csrc_digest():
+            return None, "profiles/traffic.txt is stale: the kernel sources changed after the capture (%s)" % rec.get("captured")
+        return t, "profiles/traffic.txt: ncu --set full capture of %s, kernel sources %s (not measured in this run)" % (
+            rec.get("captured"), rec.get("csrc_sha256_16"))
+    except Exception as e:      # a broken record is no record
+        return None, f"profiles/traffic.txt unreadable: {e}"
+
+
 def peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -255,6 +286,15 @@ def main():
     cells_step = 2.0 * prm.N * (prm.nt - 1)                # forward + adjoint
     value = whole_job_rate(cells_step, args.steps, world, ms)
 
+    # ---- look at what the timed steps produced: a blow-up must not print a throughput
+    d64, i64 = data.double(), image.double()
+    checks = {"finite": bool(torch.isfinite(data).all().item() and torch.isfinite(image).all().item()),
+              "data_l2": float(d64.norm().item()), "image_l2": float(i64.norm().item()),
+              "data_absmax": float(data.abs().max().item()), "image_absmax": float(image.abs().max().item())}
+    del d64, i64
+    assert checks["finite"], f"non-finite values in the result of the timed steps: {checks}"
+    assert checks["data_l2"] > 0.0 and checks["image_l2"] > 0.0, f"the timed steps produced zeros: {checks}"
+
     # ---- roofline of the step kernels, from the library's own CUDA events in the timed region
     loop_f, k_f, n_f = ctx.timing("forward")
     loop_a, k_a, n_a = ctx.timing("adjoint")
@@ -276,16 +316,13 @@ def main():
                 "adjoint_frac": B_ALG * prm.N / (t_adj * 1e-3) / 1e9 / peak,
                 "forward_loop_ms": loop_f, "adjoint_loop_ms": loop_a,
                 "kernel_ms": {"forward": {k: v for k, v in k_f.items() if v}, "adjoint": {k: v for k, v in k_a.items() if v}}}
-        tr = os.path.join(ROOT, "profiles", "r1_traffic.txt")   # per-launch DRAM bytes from the committed ncu capture
-        if os.path.exists(tr):
-            try:
-                t = json.load(open(tr)).get(f"config{args.config}")
-                # per launch of the dominant kernel (the adjoint step), from the committed ncu --set full capture
-                roof["traffic"] = t["adjoint_bytes_per_launch"] / 1e9 if t else None
-                roof["traffic_unit"] = "GB per launch (dram__bytes_read.sum + dram__bytes_write.sum), algorithmic %.2f" % (B_ALG * prm.N / 1e9)
-                roof["traffic_forward"] = t["forward_bytes_per_launch"] / 1e9 if t else None
-            except Exception:
-                pass
+        t, src = committed_traffic(args.config)
+        roof["traffic_source"] = src
+        if t:
+            # per launch of the dominant kernel (the adjoint step)
+            roof["traffic"] = t["adjoint_bytes_per_launch"] / 1e9
+            roof["traffic_unit"] = "GB per launch (dram__bytes_read.sum + dram__bytes_write.sum), algorithmic %.2f" % (B_ALG * prm.N / 1e9)
+            roof["traffic_forward"] = t["forward_bytes_per_launch"] / 1e9
 
     # ---- end to end through the host-buffer entry points (pinned host memory, copies inside)
     e2e = None
@@ -322,7 +359,8 @@ def main():
                            "step": "one pact_forward + one pact_adjoint", "l2": "inputs larger than L2 (no flush needed)"
                            if ctx.device_bytes() > 4 * 126e6 else "working set near L2 size: latency/L2-bound case",
                            "variant": args.variant, "device_bytes": ctx.device_bytes()},
-                "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clk}
+                "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clk,
+                "checks": checks}
         print(json.dumps(line), flush=True)
     ctx.close()
     if world > 1:

@@ -27,11 +27,15 @@ extern "C" {
 
 #define PACT_OK          0
 #define PACT_EINVAL     -1  /* NULL pointer, non-positive size/h/dt/nt, n < 8 or 2*npml+8 > min(nx,ny,nz), bad PML constants */
-#define PACT_ECFL       -2  /* dt * c_max > 6 h / (7 sqrt 3): the scheme is unstable (reading G11) */
+#define PACT_ECFL       -2  /* dt * c_max > 6 h / (7 sqrt 3), c_max^2 = max over nodes of (lambda+2mu)/rho: the scheme is
+                               unstable (reading G11).  A NECESSARY condition only: next to a much lighter
+                               neighbour the staggered density is below the node's, so stay a few per cent under it
+                               (the paper's and BASELINE's media run at <= 0.57 of the limit) */
 #define PACT_ERCV       -3  /* a receiver lies outside [0,(n-1)h] on some axis */
 #define PACT_EMATERIAL  -4  /* rho <= 0, mu < 0, lambda + 2 mu <= 0, alpha < 0 or a non-finite value */
 #define PACT_ENOMEM     -5  /* device or host allocation failed */
 #define PACT_ECUDA      -6  /* a CUDA call failed; pact_last_cuda_error() has the text */
+#define PACT_ENUMERIC   -7  /* option "check_finite": the result holds a NaN or an Inf (the output buffer is still written) */
 
 typedef struct pact_ctx pact_ctx;   /* opaque; owns every internal device buffer */
 
@@ -41,8 +45,8 @@ typedef struct {
     double dt;             /* time step [s] */
     int    nt;             /* = M: recorded samples p^_0 .. p^_{M-1}; M-1 applications of W' (Eq. 17) */
     int    npml;           /* C-PML thickness in cells on all six faces, inside the grid; 0 = none */
-    double pml_R;          /* theoretical reflection coefficient of the profile, in (0,1) (default 1e-4) */
-    double pml_cref;       /* reference speed of the profile [m/s] (default: max c_l) */
+    double pml_R;          /* theoretical reflection coefficient of the profile, in (0,1); 0 = default 1e-4 */
+    double pml_cref;       /* reference speed of the profile [m/s]; 0 = default: max c_l of the medium */
     double pml_beta_max;   /* CFS frequency shift beta at the PML entrance [rad/s] (Eq. 32) */
 } pact_params;
 
@@ -114,6 +118,9 @@ const char* pact_last_cuda_error(void);
  *              0: launch directly; -1: automatic.
  *   "zchunk"   planes of z each CTA of the fused kernel marches over (0 = automatic).  Any value
  *              gives the same operator; it only changes how the grid is cut into CTAs.
+ *   "check_finite"  1: pact_forward / pact_adjoint (and their _host forms) finish with a reduction over
+ *              the output, synchronise the stream and return PACT_ENUMERIC if it holds a NaN or an Inf
+ *              (a blow-up of the time stepping).  0 (default): no check, fully asynchronous.
  */
 int pact_set_option(pact_ctx* ctx, const char* key, long long value);
 

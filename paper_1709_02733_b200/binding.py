@@ -13,12 +13,11 @@ from pathlib import Path
 import numpy as np
 
 _HERE = Path(__file__).resolve().parent
-import os as _os
-_LIBPATH = Path(_os.environ.get("PACT_LIBRARY", _HERE / "libpact.so"))   # override: another build of the same library
+_LIBPATH = _HERE / "libpact.so"
 
 PACT_OK = 0
 ERRORS = {-1: "PACT_EINVAL", -2: "PACT_ECFL", -3: "PACT_ERCV", -4: "PACT_EMATERIAL", -5: "PACT_ENOMEM",
-          -6: "PACT_ECUDA"}
+          -6: "PACT_ECUDA", -7: "PACT_ENUMERIC"}
 KERNEL_KINDS = ("fwd_vel", "fwd_str", "fwd_fused", "adj_a", "adj_b", "adj_fused", "recv", "other")
 
 # every symbol include/pact.h declares (tests check that the library exports all of them)
@@ -138,22 +137,43 @@ class Pact:
     __del__ = close
 
     # ---- operators on device tensors (asynchronous on the context's stream)
+    # Results are ordered on `self.stream` (the stream the context was created with) only.  Outputs the binding
+    # allocates are allocated under that stream, inputs are recorded on it (so the caching allocator does not hand
+    # their memory out while the library still reads it), and the caller's current stream is made to wait for the
+    # library's work, so reading the result from the current stream is safe as well.
+    def _enter(self, *inputs):
+        import torch
+        cur = torch.cuda.current_stream(self.device)
+        if cur != self.stream:
+            self.stream.wait_stream(cur)          # the inputs were produced on the caller's stream
+            for t in inputs:
+                t.record_stream(self.stream)
+        return cur
+
+    def _leave(self, cur):
+        if cur != self.stream:
+            cur.wait_stream(self.stream)
+
     def forward(self, p0, out=None):
         import torch
-        if out is None:
-            out = torch.empty((self.prm.nt, self.L), dtype=torch.float32, device=self.device)
-        with torch.cuda.device(self.device):
+        cur = self._enter(p0)
+        with torch.cuda.device(self.device), torch.cuda.stream(self.stream):
+            if out is None:
+                out = torch.empty((self.prm.nt, self.L), dtype=torch.float32, device=self.device)
             _check(lib().pact_forward(self._h, _dev_f32(p0, self.shape, "p0"),
                                       _dev_f32(out, (self.prm.nt, self.L), "data")))
+        self._leave(cur)
         return out
 
     def adjoint(self, data, out=None):
         import torch
-        if out is None:
-            out = torch.empty(self.shape, dtype=torch.float32, device=self.device)
-        with torch.cuda.device(self.device):
+        cur = self._enter(data)
+        with torch.cuda.device(self.device), torch.cuda.stream(self.stream):
+            if out is None:
+                out = torch.empty(self.shape, dtype=torch.float32, device=self.device)
             _check(lib().pact_adjoint(self._h, _dev_f32(data, (self.prm.nt, self.L), "data"),
                                       _dev_f32(out, self.shape, "image")))
+        self._leave(cur)
         return out
 
     # ---- operators on host buffers (copies inside; returns when the result is in host memory)

@@ -64,6 +64,15 @@ __global__ void k_scale_materials(const float* __restrict__ lam, const float* __
     Aa[dst] = alpha ? (float)((double)alpha[src] * dt) : 0.0f;
 }
 
+// ---- option "check_finite": flag <- 1 if any of the n values is a NaN or an Inf ------------------------
+__global__ void k_check_finite(const float* __restrict__ v, long long n, unsigned int* flag)
+{
+    bool bad = false;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        bad |= !isfinite(v[i]);
+    if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) atomicOr(flag, 1u);
+}
+
 // ---- device-resident call arguments (so that captured graphs survive new user pointers) ---------
 struct IoArgs {
     const float* p0;     // pact_forward input

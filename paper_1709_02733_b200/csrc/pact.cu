@@ -82,6 +82,9 @@ struct pact_ctx {
     int variant;             // 0 auto, 1 plain, 2 tiled
     int use_graph;           // -1 auto, 0 off, 1 on
     int profile;
+    int check_finite;        // option: reduce the output of every operator call to a NaN/Inf flag (synchronises)
+    unsigned int* d_flag;    // that flag
+    int num_sms;             // cudaDevAttrMultiProcessorCount of the context's device
     cudaGraphExec_t gexec[2];     // forward / adjoint loop
     int gexec_variant[2];
     // timing of the last profiled call
@@ -169,6 +172,7 @@ extern "C" const char* pact_strerror(int code)
     case PACT_EMATERIAL: return "invalid material value";
     case PACT_ENOMEM: return "out of memory";
     case PACT_ECUDA: return "CUDA error";
+    case PACT_ENUMERIC: return "the result holds a NaN or an Inf";
     default: return "unknown error";
     }
 }
@@ -199,7 +203,13 @@ static int create_impl(pact_ctx* c, const pact_params* prm, const float* lam, co
     int rc = dev_alloc(c, (void**)&d_scan, 2 * sizeof(unsigned int));
     if (rc) return rc;
     CK(cudaMemsetAsync(d_scan, 0, 2 * sizeof(unsigned int), c->stream));
-    k_scan_materials<<<148 * 8, 256, 0, c->stream>>>(lam, mu, rho, alpha, c->N, d_scan, d_scan + 1);
+    {
+        int dev = 0;
+        CK(cudaGetDevice(&dev));
+        CK(cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev));
+        if (c->num_sms <= 0) c->num_sms = 148;
+    }
+    k_scan_materials<<<c->num_sms * 8, 256, 0, c->stream>>>(lam, mu, rho, alpha, c->N, d_scan, d_scan + 1);
     CK(cudaGetLastError());
     unsigned int h_scan[2];
     CK(cudaMemcpyAsync(h_scan, d_scan, sizeof(h_scan), cudaMemcpyDeviceToHost, c->stream));
@@ -209,6 +219,10 @@ static int create_impl(pact_ctx* c, const pact_params* prm, const float* lam, co
     float c2;
     memcpy(&c2, &h_scan[1], sizeof(float));
     const double cmax = std::sqrt((double)c2);
+    if (prm->npml > 0) {   // documented defaults of include/pact.h
+        if (c->prm.pml_R == 0.0) c->prm.pml_R = 1e-4;
+        if (c->prm.pml_cref == 0.0) c->prm.pml_cref = cmax;
+    }
     const double limit = 6.0 * prm->h / (7.0 * std::sqrt(3.0));   // DESIGN.md reading G11
     if (prm->dt * cmax > limit * (1.0 + 1e-6)) return PACT_ECFL;
 
@@ -267,8 +281,8 @@ static int create_impl(pact_ctx* c, const pact_params* prm, const float* lam, co
     for (int b = 0; b < 3; ++b) {
         const int n = b == 0 ? nx : (b == 1 ? ny : nz);
         std::vector<float> ai, bi, ah, bh;
-        cpml_profile(*prm, n, false, ai, bi);
-        cpml_profile(*prm, n, true, ah, bh);
+        cpml_profile(c->prm, n, false, ai, bi);
+        cpml_profile(c->prm, n, true, ah, bh);
         float* d;
         if ((rc = upload(c, &d, ai))) return rc; g.tab[b][T_A_INT] = d;
         if ((rc = upload(c, &d, bi))) return rc; g.tab[b][T_B_INT] = d;
@@ -310,6 +324,7 @@ static int create_impl(pact_ctx* c, const pact_params* prm, const float* lam, co
     }
     for (int k = 0; k < 9; ++k) g.scr[k] = nullptr;
 
+    if ((rc = dev_alloc(c, (void**)&c->d_flag, sizeof(unsigned int)))) return rc;
     if ((rc = dev_alloc(c, (void**)&c->d_io, sizeof(IoArgs)))) return rc;
     CK(cudaMemsetAsync(c->d_io, 0, sizeof(IoArgs), c->stream));
     for (int op = 0; op < 2; ++op)
@@ -327,9 +342,9 @@ extern "C" int pact_create(pact_ctx** out, const pact_params* prm, const float* 
     if (prm->nx < 8 || prm->ny < 8 || prm->nz < 8 || prm->nt < 1 || prm->npml < 0) return PACT_EINVAL;
     if (!(prm->h > 0.0) || !(prm->dt > 0.0) || !std::isfinite(prm->h) || !std::isfinite(prm->dt)) return PACT_EINVAL;
     if (2 * prm->npml + 8 > std::min(prm->nx, std::min(prm->ny, prm->nz))) return PACT_EINVAL;
-    if (prm->npml > 0 && (!(prm->pml_R > 0.0 && prm->pml_R < 1.0) || !(prm->pml_cref > 0.0) ||
+    if (prm->npml > 0 && (!(prm->pml_R >= 0.0 && prm->pml_R < 1.0) || !(prm->pml_cref >= 0.0) || !std::isfinite(prm->pml_cref) ||
                           !(prm->pml_beta_max >= 0.0) || !std::isfinite(prm->pml_beta_max)))
-        return PACT_EINVAL;
+        return PACT_EINVAL;   // pml_R = 0 / pml_cref = 0 select the defaults (1e-4, max c_l)
     if ((double)prm->nx * prm->ny * prm->nz > 2.0e9) return PACT_EINVAL;   // 32-bit cell counts inside kernels
     pact_ctx* c = new (std::nothrow) pact_ctx();
     if (!c) return PACT_ENOMEM;
@@ -367,12 +382,13 @@ struct Launcher {
                 c->samples[op][kind].push_back(p);
             }
             ev = &c->samples[op][kind][c->used[op][kind]++];
-            cudaEventRecord(ev->a, c->stream);
+            cudaError_t e = cudaEventRecord(ev->a, c->stream);
+            if (e != cudaSuccess) { err = cuda_fail(e, "cudaEventRecord", __LINE__); return; }
         }
         launch();
-        if (ev) cudaEventRecord(ev->b, c->stream);
-        c->launches[op][kind]++;
         cudaError_t e = cudaGetLastError();
+        if (e == cudaSuccess && ev) e = cudaEventRecord(ev->b, c->stream);
+        c->launches[op][kind]++;
         if (e != cudaSuccess) err = cuda_fail(e, "kernel launch", __LINE__);
     }
 };
@@ -385,7 +401,7 @@ static int resolve_variant(const pact_ctx* c)
     if (!c->bulk_positive) return 1;
     if (c->variant != 0) return c->variant;
     const long long bricks = (long long)((c->prm.nx + FT_TX - 1) / FT_TX) * ((c->prm.ny + FT_TY - 1) / FT_TY) * ((c->prm.nz + 31) / 32);
-    return bricks >= 148 ? 2 : 1;
+    return bricks >= c->num_sms ? 2 : 1;
 }
 
 static int ensure_scratch(pact_ctx* c)
@@ -587,7 +603,11 @@ static void fused_step(pact_ctx* c, Launcher& ln, int cur, float sgn, int kind)
     for (int k = 0; k < 18; ++k) { fa.mvi[k] = c->mvbuf[cur][k]; fa.mvo[k] = c->mvbuf[1 - cur][k]; }
     cudaStream_t st = c->stream, aux = c->aux_stream;
     const bool both = c->nwork[0] > 0 && c->nwork[1] > 0;
-    if (both) { cudaEventRecord(c->ev_fork, st); cudaStreamWaitEvent(aux, c->ev_fork, 0); }
+    if (both) {
+        cudaError_t e = cudaEventRecord(c->ev_fork, st);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(aux, c->ev_fork, 0);
+        if (e != cudaSuccess) { ln.err = cuda_fail(e, "fork to the slab stream", __LINE__); return; }
+    }
     FusedArgs fs = fa, fi = fa;
     fs.work = c->d_work[1];
     fi.work = c->d_work[0];
@@ -610,8 +630,9 @@ static void fused_step(pact_ctx* c, Launcher& ln, int cur, float sgn, int kind)
     ln.run(kind, [&] {
         launch_slab();
         launch_int();
-        cudaEventRecord(c->ev_join, aux);
-        cudaStreamWaitEvent(st, c->ev_join, 0);
+        cudaError_t e = cudaEventRecord(c->ev_join, aux);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(st, c->ev_join, 0);
+        if (e != cudaSuccess && !ln.err) ln.err = cuda_fail(e, "join of the slab stream", __LINE__);
     });
     c->launches[ln.op][PACT_K_OTHER]++;
 }
@@ -722,17 +743,33 @@ static int run_loop(pact_ctx* c, int which /*0 fwd, 1 adj*/)
     return PACT_OK;
 }
 
+// option "check_finite" (failure detection): NaN / Inf anywhere in the result -> PACT_ENUMERIC
+static int finite_check(pact_ctx* c, const float* out, long long n)
+{
+    if (!c->check_finite || n <= 0) return PACT_OK;
+    CK(cudaMemsetAsync(c->d_flag, 0, sizeof(unsigned int), c->stream));
+    k_check_finite<<<c->num_sms * 4, 256, 0, c->stream>>>(out, n, c->d_flag);
+    CK(cudaGetLastError());
+    unsigned int h = 0;
+    CK(cudaMemcpyAsync(&h, c->d_flag, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    return h ? PACT_ENUMERIC : PACT_OK;
+}
+
 extern "C" int pact_forward(pact_ctx* c, const float* p0, float* data)
 {
     if (!c || !p0 || (!data && c->L > 0)) return PACT_EINVAL;
     cudaStream_t st = c->stream;
     IoArgs io{p0, data, nullptr, nullptr};
     k_set_io<<<1, 1, 0, st>>>(c->d_io, io);
+    CK(cudaGetLastError());
     CK(cudaMemsetAsync(c->state_base, 0, (size_t)c->state_bytes, st));
     dim3 blk(64, 4), grd((c->g.nx + 63) / 64, (c->g.ny + 3) / 4, c->g.nz);
     k_inject<<<grd, blk, 0, st>>>(c->g, c->d_io);
     CK(cudaGetLastError());
-    return run_loop(c, 0);
+    int rc = run_loop(c, 0);
+    if (rc) return rc;
+    return finite_check(c, data, (long long)c->prm.nt * c->L);
 }
 
 extern "C" int pact_adjoint(pact_ctx* c, const float* data, float* image)
@@ -741,8 +778,11 @@ extern "C" int pact_adjoint(pact_ctx* c, const float* data, float* image)
     cudaStream_t st = c->stream;
     IoArgs io{nullptr, nullptr, data, image};
     k_set_io<<<1, 1, 0, st>>>(c->d_io, io);
+    CK(cudaGetLastError());
     CK(cudaMemsetAsync(c->state_base, 0, (size_t)c->state_bytes, st));
-    return run_loop(c, 1);
+    int rc = run_loop(c, 1);
+    if (rc) return rc;
+    return finite_check(c, image, c->N);
 }
 
 // ---- host-buffer variants -----------------------------------------------------------------------
@@ -759,11 +799,12 @@ extern "C" int pact_forward_host(pact_ctx* c, const float* p0_host, float* data_
     int rc = ensure_host_staging(c);
     if (rc) return rc;
     CK(cudaMemcpyAsync(c->d_vol, p0_host, (size_t)c->N * sizeof(float), cudaMemcpyHostToDevice, c->stream));
-    if ((rc = pact_forward(c, c->d_vol, c->d_dat))) return rc;
+    rc = pact_forward(c, c->d_vol, c->d_dat);
+    if (rc && rc != PACT_ENUMERIC) return rc;
     if (c->L > 0)
         CK(cudaMemcpyAsync(data_host, c->d_dat, (size_t)c->prm.nt * c->L * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
-    return PACT_OK;
+    return rc;
 }
 
 extern "C" int pact_adjoint_host(pact_ctx* c, const float* data_host, float* image_host)
@@ -773,10 +814,11 @@ extern "C" int pact_adjoint_host(pact_ctx* c, const float* data_host, float* ima
     if (rc) return rc;
     if (c->L > 0)
         CK(cudaMemcpyAsync(c->d_dat, data_host, (size_t)c->prm.nt * c->L * sizeof(float), cudaMemcpyHostToDevice, c->stream));
-    if ((rc = pact_adjoint(c, c->d_dat, c->d_vol))) return rc;
+    rc = pact_adjoint(c, c->d_dat, c->d_vol);
+    if (rc && rc != PACT_ENUMERIC) return rc;
     CK(cudaMemcpyAsync(image_host, c->d_vol, (size_t)c->N * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
-    return PACT_OK;
+    return rc;
 }
 
 // ---- options and timing -------------------------------------------------------------------------
@@ -784,6 +826,7 @@ extern "C" int pact_set_option(pact_ctx* c, const char* key, long long value)
 {
     if (!c || !key) return PACT_EINVAL;
     if (!strcmp(key, "profile")) { c->profile = value != 0; return PACT_OK; }
+    if (!strcmp(key, "check_finite")) { c->check_finite = value != 0; return PACT_OK; }
     if (!strcmp(key, "variant")) {
         if (value < 0 || value > 2) return PACT_EINVAL;
         c->variant = (int)value;
