@@ -301,8 +301,10 @@ def main():
     ctx.set_option("profile", 0)
     launches = (sum(n_f.values()) + sum(n_a.values()) + 3) * args.steps   # + argument record x2 and tau per step
     # device time of one time step's kernels (all launches of the step, in the mix they ran)
-    t_fwd = (k_f["fwd_vel"] * n_f["fwd_vel"] + k_f["fwd_str"] * n_f["fwd_str"] + k_f["fwd_fused"] * n_f["fwd_fused"]) / max(prm.nt - 1, 1)
-    t_adj = (k_a["adj_a"] * n_a["adj_a"] + k_a["adj_b"] * n_a["adj_b"] + k_a["adj_fused"] * n_a["adj_fused"]) / max(prm.nt - 1, 1)
+    step_kinds_f = ("fwd_vel", "fwd_str", "fwd_fused", "fwd_slab", "fwd_interior")
+    step_kinds_a = ("adj_a", "adj_b", "adj_fused", "adj_slab", "adj_interior")
+    t_fwd = sum(k_f[k] * n_f[k] for k in step_kinds_f) / max(prm.nt - 1, 1)
+    t_adj = sum(k_a[k] * n_a[k] for k in step_kinds_a) / max(prm.nt - 1, 1)
     peak, peak_src = peaks()
     pml_extra = 48.0 * 3 * 2 * prm.npml / prm.nx if prm.npml else 0.0
     roof = None

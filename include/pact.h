@@ -118,6 +118,10 @@ const char* pact_last_cuda_error(void);
  *              0: launch directly; -1: automatic.
  *   "zchunk"   planes of z each CTA of the fused kernel marches over (0 = automatic).  Any value
  *              gives the same operator; it only changes how the grid is cut into CTAs.
+ *   "split_launch"  1 (default): a fused time step runs its C-PML (slab) bricks and then its C-PML-free
+ *              (interior) bricks as two launches on the context's stream, each timed on its own
+ *              (PACT_K_*_SLAB / PACT_K_*_INTERIOR); 0: one persistent launch over the whole work list
+ *              (PACT_K_*_FUSED).  Same bricks, same operator, same bits (measured within 2 % of each other).
  *   "check_finite"  1: pact_forward / pact_adjoint (and their _host forms) finish with a reduction over
  *              the output, synchronise the stream and return PACT_ENUMERIC if it holds a NaN or an Inf
  *              (a blow-up of the time stepping).  0 (default): no check, fully asynchronous.
@@ -128,22 +132,25 @@ int pact_set_option(pact_ctx* ctx, const char* key, long long value);
  * pact_get_timing — timings of the LAST pact_forward (op = 0) or pact_adjoint (op = 1) call made
  * with "profile" = 1.  Synchronises the context's stream.
  *   loop_ms      [out] device time of the whole time loop (IC / read-out excluded).
- *   kernel_ms    [out] double[8]: mean device time of one launch of kernel kind k (CUDA events on
+ *   kernel_ms    [out] double[PACT_K_COUNT]: mean device time of one launch of kernel kind k (CUDA events on
  *                      the context's stream around launches sampled evenly over the loop), 0 if
  *                      that kind did not run.  Kinds: PACT_K_*.
- *   launches     [out] long long[8]: number of launches of kind k in that call.
+ *   launches     [out] long long[PACT_K_COUNT]: number of launches of kind k in that call.
  * Any output pointer may be NULL.  Errors: PACT_EINVAL (no profiled call of that op yet), PACT_ECUDA.
  */
 #define PACT_K_FWD_VEL   0   /* Eq. 46a,b */
 #define PACT_K_FWD_STR   1   /* Eq. 46c,d */
-#define PACT_K_FWD_FUSED 2   /* Eq. 46a-d in one pass (interior launch + slab launch, timed as one) */
+#define PACT_K_FWD_FUSED 2   /* Eq. 46a-d in one pass: the persistent launch of one fused time step */
 #define PACT_K_ADJ_A     3   /* Eq. 61a,b,f : sigma_bar -> u_bar, psi_bar */
 #define PACT_K_ADJ_B     4   /* Eq. 61c,d,e,g : u_bar -> sigma_bar, phi_bar */
 #define PACT_K_ADJ_FUSED 5
 #define PACT_K_RECV      6   /* Theta gather / Theta^T scatter, Eq. 56, 60 */
-#define PACT_K_OTHER     7   /* launches counted but not timed on their own: the C-PML (slab) launch of a fused
-                                step, which runs on a second stream beside the interior launch and is inside the
-                                PACT_K_*_FUSED time of that step */
+#define PACT_K_OTHER     7   /* tau^T read-out */
+#define PACT_K_FWD_SLAB      8   /* option "split_launch": the C-PML bricks of a fused forward step */
+#define PACT_K_FWD_INTERIOR  9   /*                        the C-PML-free bricks */
+#define PACT_K_ADJ_SLAB     10
+#define PACT_K_ADJ_INTERIOR 11
+#define PACT_K_COUNT        12
 int pact_get_timing(pact_ctx* ctx, int op, double* loop_ms, double* kernel_ms, long long* launches);
 
 /* Bytes of device memory owned by the context. */

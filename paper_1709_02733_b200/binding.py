@@ -18,7 +18,8 @@ _LIBPATH = _HERE / "libpact.so"
 PACT_OK = 0
 ERRORS = {-1: "PACT_EINVAL", -2: "PACT_ECFL", -3: "PACT_ERCV", -4: "PACT_EMATERIAL", -5: "PACT_ENOMEM",
           -6: "PACT_ECUDA", -7: "PACT_ENUMERIC"}
-KERNEL_KINDS = ("fwd_vel", "fwd_str", "fwd_fused", "adj_a", "adj_b", "adj_fused", "recv", "other")
+KERNEL_KINDS = ("fwd_vel", "fwd_str", "fwd_fused", "adj_a", "adj_b", "adj_fused", "recv", "other",
+                "fwd_slab", "fwd_interior", "adj_slab", "adj_interior")       # PACT_K_* of include/pact.h
 
 # every symbol include/pact.h declares (tests check that the library exports all of them)
 SYMBOLS = ("pact_create", "pact_forward", "pact_adjoint", "pact_forward_host", "pact_adjoint_host",
@@ -134,7 +135,11 @@ class Pact:
             lib().pact_destroy(self._h)
             self._h = None
 
-    __del__ = close
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:       # interpreter shutdown: module globals may already be gone
+            pass
 
     # ---- operators on device tensors (asynchronous on the context's stream)
     # Results are ordered on `self.stream` (the stream the context was created with) only.  Outputs the binding
@@ -210,8 +215,8 @@ class Pact:
         (op = 0 or "forward") or adjoint (op = 1 or "adjoint") call."""
         op = {"forward": 0, "adjoint": 1}.get(op, op)
         loop = C.c_double()
-        km = (C.c_double * 8)()
-        ln = (C.c_longlong * 8)()
+        km = (C.c_double * len(KERNEL_KINDS))()
+        ln = (C.c_longlong * len(KERNEL_KINDS))()
         _check(lib().pact_get_timing(self._h, int(op), C.byref(loop), km, ln))
         return loop.value, dict(zip(KERNEL_KINDS, km)), dict(zip(KERNEL_KINDS, ln))
 

@@ -67,16 +67,20 @@
 #define FT_OFF_XT (FT_OFF_END + 16)   // after 8 mbarriers (64 B)
 #define FT_OFF_YT (FT_OFF_XT + 4 * FT_TABW)
 #define FT_OFF_ZT (FT_OFF_YT + 4 * FT_TABW)
-#define FT_SMEM_BYTES ((FT_OFF_ZT + 4 * FT_ZRING) * 4)
+#define FT_SMEM_BYTES ((FT_OFF_ZT + 4 * FT_ZRING + 4) * 4)   // + the work-queue ticket
 
 // kernel modes: which C-PML code a launch carries (CTAs away from the slabs skip it at run time)
 #define FM_PLAIN 0     // no C-PML (npml = 0)
 #define FM_FWD 1       // W'   : Eq. 46a-d, memory variables updated after differencing
 #define FM_ADJ 2       // W'^T : Eq. 61, memory variables (tilde form) applied before differencing
 
+#define FT_WORK_SLAB 0x10000           // flag in work[b].x: the brick touches a C-PML slab (runs the launch's C-PML code)
+
 struct FusedArgs {
     int nx, ny, nz;
-    const int4* work;      // CTA b processes tile (work[b].x, work[b].y), planes [work[b].z, work[b].w)
+    const int4* work;      // brick b: tile (work[b].x & 0xffff, work[b].y), planes [work[b].z, work[b].w) ; FT_WORK_SLAB flag in .x
+    int work_begin, work_end;   // the launch processes bricks [work_begin, work_end) of the list, in list order
+    unsigned int* queue;   // [2]: next brick (relative to work_begin), CTAs that left ; both reset by the last CTA to leave
     long long sy, sz, box; // strides (elements) of the padded box; elements per field
     const float* in;       // state read  (field k at in + k*box; pointer to node (0,0,0))
     float* out;            // state written
@@ -98,6 +102,10 @@ __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)_
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
 {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_inval(uint64_t* bar)
+{
+    asm volatile("mbarrier.inval.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
 {
@@ -182,6 +190,17 @@ __device__ __forceinline__ void ldg4_into(float4& v, const float* p, bool pred)
         "}"
         : "+f"(v.x), "+f"(v.y), "+f"(v.z), "+f"(v.w)
         : "l"(p), "r"((int)pred));
+}
+// L2 prefetch of the line(s) holding the quad at p (memory variables of the next plane: their loads then hit L2
+// instead of exposing a DRAM latency per stage)
+__device__ __forceinline__ void pf_l2(const float* p, bool pred)
+{
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %1, 0;\n\t"
+        "@p prefetch.global.L2 [%0];\n\t"
+        "}" ::"l"(p), "r"((int)pred));
 }
 __device__ __forceinline__ void stg4(float* p, float4 v) { *reinterpret_cast<float4*>(p) = v; }
 
@@ -321,21 +340,18 @@ __device__ __forceinline__ float4 adj_own_x(float4 Told, float* To, long long i,
 // index algebra.  Relative plane j <-> z = zb - 2 + j ; iteration `it` computes u(kk = zb - 2 + it)
 // and sigma(ks = kk - 2).
 template <int MODE>
-__global__ void __launch_bounds__(FT_NT, 1)
-k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUtensorMap tmS36,
-        const __grid_constant__ CUtensorMap tmM37, const __grid_constant__ CUtensorMap tmM36,
-        const __grid_constant__ CUtensorMap tmL, const __grid_constant__ CUtensorMap tmS32, const FusedArgs a)
+__device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtensorMap& tmS40, const CUtensorMap& tmS36,
+                                            const CUtensorMap& tmM37, const CUtensorMap& tmM36, const CUtensorMap& tmL,
+                                            const CUtensorMap& tmS32, const FusedArgs& a, const int4 wk, const bool first)
 {
-    extern __shared__ __align__(1024) float sm[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(sm + FT_OFF_END);
     uint64_t* barG = bars;        // [2]  everything first read by stage 1 of iteration c -> slot c & 1
     uint64_t* barM = bars + 2;    // [3]  mu of plane j -> slot j % 3
     uint64_t* barU = bars + 5;    // [2]  u_old of plane c, landed in ring slot c % FT_RING -> barrier c & 1
 
     const int tid = threadIdx.x;
-    const int4 wk = __ldg(a.work + blockIdx.x);
     const int zb = wk.z, ze = wk.w;
-    const int x0 = wk.x * FT_TX, y0 = wk.y * FT_TY;
+    const int x0 = (wk.x & 0xffff) * FT_TX, y0 = wk.y * FT_TY;
     const int itn = ze - zb + 4;            // iterations: u planes kk = zb-2 .. ze+1
 
     // thread -> quad of the u region (10 quads x 36 rows)
@@ -385,8 +401,11 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
             sm[FT_OFF_ZT + t * FT_ZRING + (z & (FT_ZRING - 1))] = (unsigned)z < (unsigned)a.nz ? __ldg(a.tab[2][t] + z) : 0.0f;
         }
     }
-    if (tid == 0) {
-        for (int k = 0; k < 8; ++k) mbar_init(&bars[k], 1);
+    if (tid == 0) {   // fresh barriers per brick (every transaction of the previous brick was waited for)
+        for (int k = 0; k < 8; ++k) {
+            if (!first) mbar_inval(&bars[k]);
+            mbar_init(&bars[k], 1);
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
@@ -637,6 +656,8 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
             *reinterpret_cast<float4*>(R1) = n1;
             *reinterpret_cast<float4*>(R2) = n2;
             *reinterpret_cast<float4*>(R3) = n3;
+            // generic-proxy writes to a slot that issueU refills through the async proxy four iterations later
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             const long long g = (long long)kk * a.sz + gxy;
             if (wr1) {
                 store_quad(a.out + U1 * box + g, n1, x, a.nx);
@@ -670,6 +691,33 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
                 se2 = ok && (exa == 0 ? colq >= 0 : prow >= 0);
                 i2 = se2 ? (exa == 0 ? idx_x(a, colq, y, kk - 2) : idx_y(a, x, prow, kk - 2)) : 0;
                 ldg4_into(e2[0], a.mvi[exa] + i2, se2); ldg4_into(e2[1], a.mvi[3 + exa] + i2, se2); ldg4_into(e2[2], a.mvi[6 + exa] + i2, se2);
+            }
+        }
+        // L2 prefetch of the memory variables the next iteration reads (own quad): stage-1 arrays at plane kk + 1,
+        // stage-2 arrays at plane ks + 1 ; along z the adjoint's taps reach two planes further
+        if (MODE != FM_PLAIN && pml && (bx || by || kk - 6 < a.P || kk + 6 >= a.nz - 1 - a.P)) {
+            const int S1 = MODE == FM_ADJ ? 9 : 0, S2 = 9 - S1, zq = MODE == FM_ADJ ? 2 : 0;
+            {
+                const int z1 = kk + 1;
+                const bool ok = pok && (unsigned)z1 < (unsigned)a.nz;
+                const bool ex = ok && colq >= 0, ey = ok && prow >= 0;
+                const int pzr = pok ? yzslab_row(z1 + zq, a.nz, a.P) : -1;
+                const bool ez = pzr >= 0;
+                const long long ix = ex ? idx_x(a, colq, y, z1) : 0, iy = ey ? idx_y(a, x, prow, z1) : 0, iz = ez ? idx_z(a, x, y, pzr) : 0;
+                pf_l2(a.mvi[S1 + 0] + ix, ex); pf_l2(a.mvi[S1 + 3] + ix, ex); pf_l2(a.mvi[S1 + 6] + ix, ex);
+                pf_l2(a.mvi[S1 + 1] + iy, ey); pf_l2(a.mvi[S1 + 4] + iy, ey); pf_l2(a.mvi[S1 + 7] + iy, ey);
+                pf_l2(a.mvi[S1 + 2] + iz, ez); pf_l2(a.mvi[S1 + 5] + iz, ez); pf_l2(a.mvi[S1 + 8] + iz, ez);
+            }
+            {
+                const int z2 = kk - 1;
+                const bool ok = inner && (unsigned)z2 < (unsigned)a.nz;
+                const bool ex = ok && colq >= 0, ey = ok && prow >= 0;
+                const int pzr = inner ? yzslab_row(z2 + zq, a.nz, a.P) : -1;
+                const bool ez = pzr >= 0;
+                const long long ix = ex ? idx_x(a, colq, y, z2) : 0, iy = ey ? idx_y(a, x, prow, z2) : 0, iz = ez ? idx_z(a, x, y, pzr) : 0;
+                pf_l2(a.mvi[S2 + 0] + ix, ex); pf_l2(a.mvi[S2 + 3] + ix, ex); pf_l2(a.mvi[S2 + 6] + ix, ex);
+                pf_l2(a.mvi[S2 + 1] + iy, ey); pf_l2(a.mvi[S2 + 4] + iy, ey); pf_l2(a.mvi[S2 + 7] + iy, ey);
+                pf_l2(a.mvi[S2 + 2] + iz, ez); pf_l2(a.mvi[S2 + 5] + iz, ez); pf_l2(a.mvi[S2 + 8] + iz, ez);
             }
         }
         if (pml && tid >= 360 && tid < 364) {   // z table ring: plane kk + 3 (first read after the barrier)
@@ -832,5 +880,43 @@ k_fused(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUten
         w13a = w13b; w13b = w13c; w13c = f13;
         w23a = w23b; w23b = w23c; w23c = f23;
         w33a = w33b; w33b = w33c; w33c = w33d; w33d = f33;
+    }
+}
+
+// =================================================================================================
+// One launch = one time step.  The launch is persistent: one CTA per SM pulls bricks off the work list through
+// an atomic counter, heaviest first (host order: C-PML bricks, then long interior bricks, short ones last), so
+// that no SM idles while another still holds a long brick and no wave of CTAs ends on a partial wave.  Bricks
+// flagged FT_WORK_SLAB run the launch's C-PML code (MODE), the others the C-PML-free instance of the same
+// brick routine.  The last CTA to leave resets the queue for the next launch.
+template <int MODE>
+__global__ void __launch_bounds__(FT_NT, 1)
+k_step(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUtensorMap tmS36,
+       const __grid_constant__ CUtensorMap tmM37, const __grid_constant__ CUtensorMap tmM36,
+       const __grid_constant__ CUtensorMap tmL, const __grid_constant__ CUtensorMap tmS32, const FusedArgs a)
+{
+    extern __shared__ __align__(1024) float sm[];
+    int* s_next = reinterpret_cast<int*>(sm + FT_OFF_ZT + 4 * FT_ZRING);
+    const int n = a.work_end - a.work_begin;
+    bool first = true;
+    for (;;) {
+        if (threadIdx.x == 0) *s_next = (int)atomicAdd(a.queue, 1u);
+        __syncthreads();                 // also: every thread is done with the previous brick's shared memory
+        const int b = *s_next;
+        if (b >= n) break;
+        const int4 wk = __ldg(a.work + a.work_begin + b);
+        if (MODE != FM_PLAIN && (wk.x & FT_WORK_SLAB)) fused_brick<MODE>(sm, tmS40, tmS36, tmM37, tmM36, tmL, tmS32, a, wk, first);
+        else fused_brick<FM_PLAIN>(sm, tmS40, tmS36, tmM37, tmM36, tmL, tmS32, a, wk, first);
+        first = false;
+        // generic-proxy writes of this brick (tables, exchange planes) precede the TMA writes of the next one
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncthreads();                 // *s_next is read by all before thread 0 overwrites it
+    }
+    if (threadIdx.x == 0) {
+        __threadfence();
+        if (atomicAdd(a.queue + 1, 1u) == gridDim.x - 1) {   // every CTA has drawn its last (out of range) ticket
+            a.queue[0] = 0u;
+            a.queue[1] = 0u;
+        }
     }
 }

@@ -66,14 +66,14 @@ struct pact_ctx {
     CUtensorMap tmS40[2], tmS36[2], tmS32[2], tmM37, tmM36, tmL;
     FusedArgs fa;
     int zchunk;              // planes per CTA along z (0 = auto)
-    // work lists of the fused launches: [0] CTAs whose bricks (with every tap of the adjoint) stay clear of the
-    // C-PML slabs (run without any C-PML code), [1] all the others
-    int4* d_work[2];
-    int nwork[2];
-    int work_zc;             // zchunk value the lists were built for (-1 = not built)
+    // work list of the fused launch, heaviest first: [0, nslab) bricks that touch a C-PML slab (they run the C-PML
+    // code), [nslab, nwork) bricks whose every tap (those of the adjoint included) stays clear of the slabs
+    int4* d_work;
+    int nwork, nslab;
+    int work_zc;             // zchunk value the list was built for (-1 = not built)
     long long work_cap;
-    cudaStream_t aux_stream; // the slab CTAs run beside the interior ones
-    cudaEvent_t ev_fork, ev_join;
+    unsigned int* d_queue;   // [2] ticket counter + exit counter of the persistent launch
+    int split_launch;        // diagnostic option: slab bricks and interior bricks as two launches, timed apart
     float* mvbuf[2][18];     // fused memory variables, two sets (read / written alternate every step)
     // host-buffer variants
     float* d_vol;            // [N]
@@ -90,9 +90,9 @@ struct pact_ctx {
     // timing of the last profiled call
     // timing of the last profiled forward ([0]) / adjoint ([1]) call
     cudaEvent_t ev_loop[2][2];
-    std::vector<EvPair> samples[2][8];
-    size_t used[2][8];
-    long long launches[2][8];
+    std::vector<EvPair> samples[2][PACT_K_COUNT];
+    size_t used[2][PACT_K_COUNT];
+    long long launches[2][PACT_K_COUNT];
     bool have_timing[2];
 };
 
@@ -150,11 +150,8 @@ extern "C" void pact_destroy(pact_ctx* c)
     cudaStreamSynchronize(c->stream);
     free_graphs(c);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
-    if (c->aux_stream) cudaStreamDestroy(c->aux_stream);
-    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
-    if (c->ev_join) cudaEventDestroy(c->ev_join);
     for (int op = 0; op < 2; ++op) {
-        for (int k = 0; k < 8; ++k)
+        for (int k = 0; k < PACT_K_COUNT; ++k)
             for (auto& s : c->samples[op][k]) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
         for (int k = 0; k < 2; ++k) if (c->ev_loop[op][k]) cudaEventDestroy(c->ev_loop[op][k]);
     }
@@ -352,6 +349,7 @@ extern "C" int pact_create(pact_ctx** out, const pact_params* prm, const float* 
     c->stream = (cudaStream_t)cuda_stream;
     c->variant = 0;
     c->use_graph = -1;
+    c->split_launch = 1;
     int rc = create_impl(c, prm, lam, mu, rho, alpha, rcv_xyz, L);
     if (rc != PACT_OK) { pact_destroy(c); return rc; }
     *out = c;
@@ -522,49 +520,54 @@ static int ensure_fused(pact_ctx* c)
     if ((rc = make_map(c, enc, &c->tmM37, baseM, 4, FT_BW, FT_RH))) return rc;
     if ((rc = make_map(c, enc, &c->tmL, baseM, 4, FT_TX, FT_TY))) return rc;
     if ((rc = make_map(c, enc, &c->tmM36, baseM, 4, FT_MW, FT_MH))) return rc;
-    CK(cudaFuncSetAttribute(k_fused<FM_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
-    CK(cudaFuncSetAttribute(k_fused<FM_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
-    CK(cudaFuncSetAttribute(k_fused<FM_ADJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
+    CK(cudaFuncSetAttribute(k_step<FM_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
+    CK(cudaFuncSetAttribute(k_step<FM_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
+    CK(cudaFuncSetAttribute(k_step<FM_ADJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
     fa.mat = g.Ll;
     c->work_zc = -1;
     c->work_cap = (long long)((g.nx + FT_TX - 1) / FT_TX) * ((g.ny + FT_TY - 1) / FT_TY) * (2 * g.nz + 2);   // worst case: one-plane chunks
-    for (int k = 0; k < 2; ++k)
-        if ((rc = dev_alloc(c, (void**)&c->d_work[k], (size_t)c->work_cap * sizeof(int4)))) return rc;
-    CK(cudaStreamCreateWithFlags(&c->aux_stream, cudaStreamNonBlocking));
-    CK(cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
-    CK(cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
+    if ((rc = dev_alloc(c, (void**)&c->d_work, (size_t)c->work_cap * sizeof(int4)))) return rc;
+    if ((rc = dev_alloc(c, (void**)&c->d_queue, 2 * sizeof(unsigned int)))) return rc;
+    CK(cudaMemsetAsync(c->d_queue, 0, 2 * sizeof(unsigned int), c->stream));
+    fa.queue = c->d_queue;
     c->fused_ready = true;
     return PACT_OK;
 }
 
-// z chunks of [z0, z1) for `tiles` tiles: `zc` planes each, or (zc <= 0) the chunk count that minimises
-// waves x (planes per chunk + 4 start-up planes) for one CTA per SM, chunks no shorter than 32 planes
-static int chunk_len(int z0, int z1, long long tiles, int zc)
+// z chunks of the plane range [z0, z1).  zc > 0: `zc` planes each (tests).  Automatic: the
+// persistent launch hands bricks out dynamically, so what matters is (a) few start-up planes (4 per brick, plus the
+// pipeline prologue) and (b) a short tail: about five sixths of the range in long chunks (<= FT_CHUNK_LONG planes),
+// the rest in short ones (<= FT_CHUNK_SHORT) that the host lists last.
+#define FT_CHUNK_LONG 128
+#define FT_CHUNK_SHORT 40
+static void cut_chunks(int z0, int z1, int zc, std::vector<std::pair<int, int>>& longs, std::vector<std::pair<int, int>>& shorts)
 {
     const int n = z1 - z0;
-    if (n <= 0) return 1;
-    if (zc > 0) return std::min(zc, n);
-    long long best = -1;
-    int len = n;
-    for (int k = 1; k <= std::max(1, n / 32); ++k) {
-        const int z = (n + k - 1) / k;
-        const long long ctas = tiles * ((n + z - 1) / z);
-        const long long cost = ((ctas + 147) / 148) * (z + 4);
-        if (best < 0 || cost < best) { best = cost; len = z; }
-    }
-    return len;
+    if (n <= 0) return;
+    auto equal_parts = [](int a, int b, int maxlen, std::vector<std::pair<int, int>>& out) {
+        const int m = b - a;
+        if (m <= 0) return;
+        const int k = (m + maxlen - 1) / maxlen;
+        for (int i = 0; i < k; ++i) out.push_back({a + (int)((long long)m * i / k), a + (int)((long long)m * (i + 1) / k)});
+    };
+    if (zc > 0) { equal_parts(z0, z1, zc, longs); return; }
+    if (n <= FT_CHUNK_SHORT + 8) { shorts.push_back({z0, z1}); return; }
+    const int tail = std::max(n / 6, 24);
+    equal_parts(z0, z1 - tail, FT_CHUNK_LONG, longs);
+    equal_parts(z1 - tail, z1, FT_CHUNK_SHORT, shorts);
 }
 
-// Work lists: a brick is "interior" when its u region with the +-2 taps of the
-// transposed C-PML recursion (x0-4 .. x0+35, likewise y, planes zb-4 .. ze+2) misses every slab; such bricks
-// run the kernel without C-PML code.  Everything else (boundary tiles over all z; the z slabs of interior
-// tiles) runs the C-PML kernel on a second stream beside it.
+// Work list: a brick is "interior" when its u region with the +-2 taps of the transposed
+// C-PML recursion (x0-4 .. x0+35, likewise y, planes zb-4 .. ze+2) misses every slab; such bricks run the brick
+// routine without C-PML code.  Everything else (boundary tiles over all z; the z slabs of interior tiles) carries
+// the FT_WORK_SLAB flag.  Order = the order the persistent launch hands them out: slab bricks first (they cost
+// about twice as much per plane), long before short, and chunk-major inside a class so that neighbouring tiles
+// march the same planes together (their shared box rows then meet in L2).
 static int build_work(pact_ctx* c)
 {
     if (c->work_zc == c->zchunk) return PACT_OK;
     const DevGrid& g = c->g;
     const int P = g.P, ntx = (g.nx + FT_TX - 1) / FT_TX, nty = (g.ny + FT_TY - 1) / FT_TY;
-    std::vector<int4> wl[2];
     auto interior_1d = [&](int t0, int n) { return P == 0 || (t0 - 4 >= P && t0 + 36 <= n - 1 - P); };
     int zlo = 0, zhi = g.nz;
     if (P > 0) { zlo = P + 4; zhi = g.nz - 5 - P; }
@@ -572,27 +575,34 @@ static int build_work(pact_ctx* c)
     for (int ty = 0; ty < nty; ++ty)
         for (int tx = 0; tx < ntx; ++tx)
             ((interior_1d(tx * FT_TX, g.nx) && interior_1d(ty * FT_TY, g.ny) && zhi - zlo >= 8) ? tin : tbd).push_back({tx, ty});
-    auto add = [&](std::vector<int4>& w, const std::vector<std::pair<int, int>>& tiles, int z0, int z1) {
-        if (tiles.empty() || z1 <= z0) return;
-        const int len = chunk_len(z0, z1, (long long)tiles.size(), c->zchunk);
-        for (int zb = z0; zb < z1; zb += len)               // chunk-major: neighbouring tiles march the same planes together
-            for (auto& t : tiles) w.push_back(make_int4(t.first, t.second, zb, std::min(zb + len, z1)));
+    std::vector<int4> wl;
+    auto add = [&](const std::vector<std::pair<int, int>>& tiles, const std::vector<std::pair<int, int>>& chunks, int flag) {
+        for (auto& ch : chunks)
+            for (auto& t : tiles) wl.push_back(make_int4(t.first | flag, t.second, ch.first, ch.second));
     };
-    add(wl[0], tin, zlo, zhi);
-    add(wl[1], tbd, 0, g.nz);
-    if (P > 0) { add(wl[1], tin, 0, zlo); add(wl[1], tin, zhi, g.nz); }
-    for (int k = 0; k < 2; ++k) {
-        if ((long long)wl[k].size() > c->work_cap) return PACT_EINVAL;
-        c->nwork[k] = (int)wl[k].size();
-        if (!wl[k].empty())
-            CK(cudaMemcpyAsync(c->d_work[k], wl[k].data(), wl[k].size() * sizeof(int4), cudaMemcpyHostToDevice, c->stream));
+    std::vector<std::pair<int, int>> bl, bs, il, is, zl, zs;
+    if (!tbd.empty()) cut_chunks(0, g.nz, c->zchunk, bl, bs);
+    if (!tin.empty()) {
+        cut_chunks(zlo, zhi, c->zchunk, il, is);
+        if (P > 0) {   // the z slabs of interior tiles: thin bricks
+            cut_chunks(0, zlo, c->zchunk, zl, zs);
+            cut_chunks(zhi, g.nz, c->zchunk, zl, zs);
+        }
     }
-    CK(cudaStreamSynchronize(c->stream));   // the vectors are temporaries
+    const int slab = P > 0 ? FT_WORK_SLAB : 0;
+    add(tbd, bl, slab); add(tbd, bs, slab); add(tin, zl, slab); add(tin, zs, slab);
+    c->nslab = P > 0 ? (int)wl.size() : 0;
+    add(tin, il, 0); add(tin, is, 0);
+    if ((long long)wl.size() > c->work_cap) return PACT_EINVAL;
+    c->nwork = (int)wl.size();
+    if (!wl.empty()) CK(cudaMemcpyAsync(c->d_work, wl.data(), wl.size() * sizeof(int4), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaStreamSynchronize(c->stream));   // the vector is a temporary
     c->work_zc = c->zchunk;
     return PACT_OK;
 }
 
-// one time step cur -> 1-cur ; sgn = +1: W' ; sgn = -1: W'^T on the scaled adjoint variables
+// one time step cur -> 1-cur ; sgn = +1: W' ; sgn = -1: W'^T on the scaled adjoint variables.  One persistent
+// launch (option "split_launch": the slab bricks and the interior bricks as two launches, each with its own events)
 static void fused_step(pact_ctx* c, Launcher& ln, int cur, float sgn, int kind)
 {
     FusedArgs fa = c->fa;
@@ -600,41 +610,24 @@ static void fused_step(pact_ctx* c, Launcher& ln, int cur, float sgn, int kind)
     const DevGrid& go = cur ? c->g : c->g2;
     fa.in = gi.f[0]; fa.out = go.f[0];
     fa.sgn = sgn;
+    fa.work = c->d_work;
     for (int k = 0; k < 18; ++k) { fa.mvi[k] = c->mvbuf[cur][k]; fa.mvo[k] = c->mvbuf[1 - cur][k]; }
-    cudaStream_t st = c->stream, aux = c->aux_stream;
-    const bool both = c->nwork[0] > 0 && c->nwork[1] > 0;
-    if (both) {
-        cudaError_t e = cudaEventRecord(c->ev_fork, st);
-        if (e == cudaSuccess) e = cudaStreamWaitEvent(aux, c->ev_fork, 0);
-        if (e != cudaSuccess) { ln.err = cuda_fail(e, "fork to the slab stream", __LINE__); return; }
-    }
-    FusedArgs fs = fa, fi = fa;
-    fs.work = c->d_work[1];
-    fi.work = c->d_work[0];
-    cudaStream_t s1 = both ? aux : st;
-    auto launch_slab = [&] {
-        const int grid = c->nwork[1];
-        if (fa.P == 0) k_fused<FM_PLAIN><<<grid, FT_NT, FT_SMEM_BYTES, s1>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fs);
-        else if (sgn > 0.0f) k_fused<FM_FWD><<<grid, FT_NT, FT_SMEM_BYTES, s1>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fs);
-        else k_fused<FM_ADJ><<<grid, FT_NT, FT_SMEM_BYTES, s1>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fs);
+    cudaStream_t st = c->stream;
+    auto launch = [&](int b0, int b1) {
+        if (b1 <= b0) return;
+        fa.work_begin = b0; fa.work_end = b1;
+        const int grid = std::min(c->num_sms, b1 - b0);
+        if (fa.P == 0) k_step<FM_PLAIN><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fa);
+        else if (sgn > 0.0f) k_step<FM_FWD><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fa);
+        else k_step<FM_ADJ><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fa);
     };
-    auto launch_int = [&] {
-        k_fused<FM_PLAIN><<<c->nwork[0], FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fi);
-    };
-    if (!both) {
-        if (c->nwork[1] > 0) ln.run(kind, launch_slab);
-        if (c->nwork[0] > 0) ln.run(kind, launch_int);
+    if (!c->split_launch || c->nslab == 0 || c->nslab == c->nwork) {
+        ln.run(kind, [&] { launch(0, c->nwork); });
         return;
     }
-    // both: timed as one (they overlap); the slab launch is counted under PACT_K_OTHER
-    ln.run(kind, [&] {
-        launch_slab();
-        launch_int();
-        cudaError_t e = cudaEventRecord(c->ev_join, aux);
-        if (e == cudaSuccess) e = cudaStreamWaitEvent(st, c->ev_join, 0);
-        if (e != cudaSuccess && !ln.err) ln.err = cuda_fail(e, "join of the slab stream", __LINE__);
-    });
-    c->launches[ln.op][PACT_K_OTHER]++;
+    const int k_slab = sgn > 0.0f ? PACT_K_FWD_SLAB : PACT_K_ADJ_SLAB, k_int = sgn > 0.0f ? PACT_K_FWD_INTERIOR : PACT_K_ADJ_INTERIOR;
+    ln.run(k_slab, [&] { launch(0, c->nslab); });
+    ln.run(k_int, [&] { launch(c->nslab, c->nwork); });
 }
 
 // Eq. 58 right to left: tau, then for m = 0..M-1 { Theta ; W' unless m = M-1 }
@@ -710,7 +703,7 @@ static int run_loop(pact_ctx* c, int which /*0 fwd, 1 adj*/)
         if ((rc = build_work(c))) return rc;
         CK(cudaMemsetAsync(c->stateB_base, 0, (size_t)c->stateB_bytes, c->stream));
     }
-    for (int k = 0; k < 8; ++k) { c->used[which][k] = 0; c->launches[which][k] = 0; }
+    for (int k = 0; k < PACT_K_COUNT; ++k) { c->used[which][k] = 0; c->launches[which][k] = 0; }
     c->have_timing[which] = c->profile != 0;
     if (want_graph(c)) {
         if (c->gexec[which] && c->gexec_variant[which] != variant) {
@@ -834,6 +827,7 @@ extern "C" int pact_set_option(pact_ctx* c, const char* key, long long value)
     }
     if (!strcmp(key, "zchunk")) { if (value < 0) return PACT_EINVAL; c->zchunk = (int)value; free_graphs(c); return PACT_OK; }
     if (!strcmp(key, "graph")) { c->use_graph = value < 0 ? -1 : (value != 0); return PACT_OK; }
+    if (!strcmp(key, "split_launch")) { c->split_launch = value != 0; free_graphs(c); return PACT_OK; }
     return PACT_EINVAL;
 }
 
@@ -846,7 +840,7 @@ extern "C" int pact_get_timing(pact_ctx* c, int op, double* loop_ms, double* ker
         CK(cudaEventElapsedTime(&ms, c->ev_loop[op][0], c->ev_loop[op][1]));
         *loop_ms = ms;
     }
-    for (int k = 0; k < 8; ++k) {
+    for (int k = 0; k < PACT_K_COUNT; ++k) {
         if (kernel_ms) {
             double acc = 0.0;
             for (size_t s = 0; s < c->used[op][k]; ++s) {
