@@ -269,6 +269,10 @@ def main():
     for _ in range(args.warmup):
         step()
     barrier()
+    try:        # homogeneous (tile, plane) material boxes served from L2-resident palette planes (fused path only)
+        elided = ctx.info("elided_material_planes")
+    except Exception:
+        elided = None
     ctx.set_option("profile", 1)         # CUDA events around sampled launches, on the library's stream
     clocks = ClockSampler(local)
     if rank == 0:
@@ -293,7 +297,8 @@ def main():
               "data_absmax": float(data.abs().max().item()), "image_absmax": float(image.abs().max().item())}
     del d64, i64
     assert checks["finite"], f"non-finite values in the result of the timed steps: {checks}"
-    assert checks["data_l2"] > 0.0 and checks["image_l2"] > 0.0, f"the timed steps produced zeros: {checks}"
+    if args.nt is None:      # (a truncated development run may end before the wave reaches a receiver)
+        assert checks["data_l2"] > 0.0 and checks["image_l2"] > 0.0, f"the timed steps produced zeros: {checks}"
 
     # ---- roofline of the step kernels, from the library's own CUDA events in the timed region
     loop_f, k_f, n_f = ctx.timing("forward")
@@ -360,7 +365,8 @@ def main():
                 "config": {"workload": workload_name(prob, args), "parallelism": "replicas only" if world > 1 else "single GPU",
                            "step": "one pact_forward + one pact_adjoint", "l2": "inputs larger than L2 (no flush needed)"
                            if ctx.device_bytes() > 4 * 126e6 else "working set near L2 size: latency/L2-bound case",
-                           "variant": args.variant, "device_bytes": ctx.device_bytes()},
+                           "variant": args.variant, "device_bytes": ctx.device_bytes(),
+                           "elided_material_planes": elided},
                 "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clk,
                 "checks": checks}
         print(json.dumps(line), flush=True)

@@ -96,6 +96,31 @@ int pact_adjoint(pact_ctx* ctx, const float* data, float* image);
 int pact_forward_host(pact_ctx* ctx, const float* p0_host, float* data_host);
 int pact_adjoint_host(pact_ctx* ctx, const float* data_host, float* image_host);
 
+/*
+ * pact_pgd — projected-gradient reconstruction with the pair, the use the paper builds it for (
+ * BASELINE config 5):  p_{k+1} = P(p_k - step * H^T (H p_k - data)),  k = 0 .. iters-1,  P = max(0, .) if nonneg
+ * else the identity.  Each iteration is one pact_forward, a fused residual kernel, one pact_adjoint and a fused
+ * update-and-clamp kernel; nothing leaves the device inside the loop.
+ *   p          [in/out] DEVICE float[nz][ny][nx]: p_0 on entry, p_iters on return.
+ *   data       [in]  DEVICE float[nt][L].
+ *   step       > 0; 1 / ||H||^2 (pact_power_iteration) makes the iteration non-expansive.
+ *   resid_l2   [out] HOST double[iters] or NULL: ||H p_k - data||_2 of every iteration (fp64 accumulation,
+ *              bit-reproducible).
+ *   update_l2  [out] HOST double[iters] or NULL: ||p_{k+1} - p_k||_2.
+ * Synchronises the stream once, at the end.  Errors: PACT_EINVAL, PACT_ENOMEM, PACT_ECUDA, PACT_ENUMERIC (option).
+ */
+int pact_pgd(pact_ctx* ctx, float* p, const float* data, double step, int iters, int nonneg,
+             double* resid_l2, double* update_l2);
+
+/*
+ * pact_power_iteration — largest eigenvalue of H^T H, i.e. ||H||^2, by `iters` power iterations.
+ *   v       [in/out] DEVICE float[nz][ny][nx]: non-zero start vector (the caller's seeded random numbers); on
+ *           return the normalised iterate (approximate dominant right singular vector of H).
+ *   sigma2  [out] HOST: ||H^T H v|| for the last normalised v.
+ * Synchronises the stream.  Errors: PACT_EINVAL, PACT_ENOMEM, PACT_ECUDA, PACT_ENUMERIC (the result is not finite).
+ */
+int pact_power_iteration(pact_ctx* ctx, float* v, int iters, double* sigma2);
+
 /* pact_destroy — free the context and everything it owns; NULL is allowed. */
 void pact_destroy(pact_ctx* ctx);
 
@@ -122,6 +147,9 @@ const char* pact_last_cuda_error(void);
  *              (interior) bricks as two launches on the context's stream, each timed on its own
  *              (PACT_K_*_SLAB / PACT_K_*_INTERIOR); 0: one persistent launch over the whole work list
  *              (PACT_K_*_FUSED).  Same bricks, same operator, same bits (measured within 2 % of each other).
+ *   "material_elision"  1 (default): the fused path fetches (tile, plane) material boxes that are one constant
+ *              4-tuple (water around a skull) from an L2-resident palette plane instead of HBM; 0: always the
+ *              real plane.  Bit-identical results.
  *   "check_finite"  1: pact_forward / pact_adjoint (and their _host forms) finish with a reduction over
  *              the output, synchronise the stream and return PACT_ENUMERIC if it holds a NaN or an Inf
  *              (a blow-up of the time stepping).  0 (default): no check, fully asynchronous.
@@ -155,6 +183,15 @@ int pact_get_timing(pact_ctx* ctx, int op, double* loop_ms, double* kernel_ms, l
 
 /* Bytes of device memory owned by the context. */
 long long pact_device_bytes(const pact_ctx* ctx);
+
+/*
+ * pact_get_info — read-only facts about a context.  Keys:
+ *   "elided_material_planes"  fraction of the fused path's (32 x 32 tile, z plane) material boxes that are
+ *                             homogeneous and served from a palette plane (builds the fused path's tables)
+ *   "num_sms"                 multiprocessors of the context's device
+ * Errors: PACT_EINVAL (NULL or unknown key), PACT_ENOMEM, PACT_ECUDA.
+ */
+int pact_get_info(pact_ctx* ctx, const char* key, double* value);
 
 #ifdef __cplusplus
 }

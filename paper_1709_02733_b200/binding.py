@@ -24,7 +24,7 @@ KERNEL_KINDS = ("fwd_vel", "fwd_str", "fwd_fused", "adj_a", "adj_b", "adj_fused"
 # every symbol include/pact.h declares (tests check that the library exports all of them)
 SYMBOLS = ("pact_create", "pact_forward", "pact_adjoint", "pact_forward_host", "pact_adjoint_host",
            "pact_destroy", "pact_strerror", "pact_last_cuda_error", "pact_set_option", "pact_get_timing",
-           "pact_device_bytes")
+           "pact_device_bytes", "pact_get_info", "pact_pgd", "pact_power_iteration")
 
 
 class PactParams(C.Structure):
@@ -68,6 +68,12 @@ def lib():
         L.pact_get_timing.argtypes = [vp, ip, C.POINTER(C.c_double), C.POINTER(C.c_double), C.POINTER(ll)]
         L.pact_device_bytes.restype = ll
         L.pact_device_bytes.argtypes = [vp]
+        L.pact_pgd.restype = ip
+        L.pact_pgd.argtypes = [vp, vp, vp, C.c_double, ip, ip, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.pact_power_iteration.restype = ip
+        L.pact_power_iteration.argtypes = [vp, vp, ip, C.POINTER(C.c_double)]
+        L.pact_get_info.restype = ip
+        L.pact_get_info.argtypes = [vp, C.c_char_p, C.POINTER(C.c_double)]
         _lib = L
     return _lib
 
@@ -181,6 +187,30 @@ class Pact:
         self._leave(cur)
         return out
 
+    # ---- projected-gradient reconstruction (pact_pgd / pact_power_iteration): marshalling only
+    def pgd(self, p, data, step, iters, nonneg=True):
+        """In place on `p`: `iters` steps of p <- max(0, p - step H^T (H p - data)).  Returns
+        (residual norms, update norms), one entry per iteration."""
+        import torch
+        cur = self._enter(p, data)
+        res = (C.c_double * max(iters, 1))()
+        upd = (C.c_double * max(iters, 1))()
+        with torch.cuda.device(self.device), torch.cuda.stream(self.stream):
+            _check(lib().pact_pgd(self._h, _dev_f32(p, self.shape, "p"), _dev_f32(data, (self.prm.nt, self.L), "data"),
+                                  float(step), int(iters), int(bool(nonneg)), res, upd))
+        self._leave(cur)
+        return list(res)[:iters], list(upd)[:iters]
+
+    def power_iteration(self, v, iters=8):
+        """||H||^2 estimate; `v` (non-zero start vector) is overwritten by the normalised iterate."""
+        import torch
+        cur = self._enter(v)
+        s2 = C.c_double()
+        with torch.cuda.device(self.device), torch.cuda.stream(self.stream):
+            _check(lib().pact_power_iteration(self._h, _dev_f32(v, self.shape, "v"), int(iters), C.byref(s2)))
+        self._leave(cur)
+        return s2.value
+
     # ---- operators on host buffers (copies inside; returns when the result is in host memory)
     def forward_host(self, p0_host, data_host):
         self._host_ok(p0_host, self.shape, "p0_host")
@@ -219,6 +249,11 @@ class Pact:
         ln = (C.c_longlong * len(KERNEL_KINDS))()
         _check(lib().pact_get_timing(self._h, int(op), C.byref(loop), km, ln))
         return loop.value, dict(zip(KERNEL_KINDS, km)), dict(zip(KERNEL_KINDS, ln))
+
+    def info(self, key):
+        v = C.c_double()
+        _check(lib().pact_get_info(self._h, key.encode(), C.byref(v)))
+        return v.value
 
     def device_bytes(self):
         return int(lib().pact_device_bytes(self._h))

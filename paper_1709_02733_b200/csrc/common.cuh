@@ -13,6 +13,7 @@
 #define PACT_HALO_X 32
 #define PACT_HALO_Y 4
 #define PACT_HALO_Z 4
+#define PACT_NPAL 4     // palette planes behind every material volume (kernels_fused.cuh, material elision)
 
 // state field order
 enum { U1 = 0, U2, U3, S11, S22, S33, S23, S13, S12, NFIELD };

@@ -84,7 +84,12 @@ struct FusedArgs {
     long long sy, sz, box; // strides (elements) of the padded box; elements per field
     const float* in;       // state read  (field k at in + k*box; pointer to node (0,0,0))
     float* out;            // state written
-    const float* mat;      // scaled materials Ll, Mi, Rr, Aa at mat + k*box (node (0,0,0))
+    // Material elision: mflag[(tile y * ntx + tile x) * nzp + z + HALO_Z] is
+    // 0, or 1 + p when all four scaled materials are constant over the tile's whole box on plane z and equal palette
+    // entry p; such planes are fetched from palette plane p (padded z index mpal + p: the same bytes, always in L2)
+    // instead of their own plane in HBM.  NULL = no elision.
+    const unsigned char* mflag;
+    int ntx, nzp, mpal;
     float sgn;             // +1: W' on (u, sigma) ; -1: W'^T on the scaled adjoint variables
     // C-PML
     int P;
@@ -136,17 +141,40 @@ __device__ __forceinline__ void tma_plane(const CUtensorMap* tm, float* dst, uin
 __device__ __forceinline__ float4 ld4s(const float* p, int quad) { return *reinterpret_cast<const float4*>(p + 4 * quad); }
 __device__ __forceinline__ float2 ld2s(const float* p, int off) { return *reinterpret_cast<const float2*>(p + off); }
 __device__ __forceinline__ float4 f4(float v) { return make_float4(v, v, v, v); }
-__device__ __forceinline__ float4 operator+(float4 a, float4 b) { return make_float4(a.x + b.x, a.y + b.y, a.z + b.z, a.w + b.w); }
-__device__ __forceinline__ float4 operator*(float4 a, float4 b) { return make_float4(a.x * b.x, a.y * b.y, a.z * b.z, a.w * b.w); }
-__device__ __forceinline__ float4 operator*(float a, float4 b) { return make_float4(a * b.x, a * b.y, a * b.z, a * b.w); }
+// Packed fp32 arithmetic of sm_100 (PTX add/sub/mul/fma .f32x2 -> SASS FADD2 / FMUL2 / FFMA2): one instruction works on
+// an aligned register pair, i.e. on half a quad, with the rounding of the scalar instruction.  The step kernels are
+// bound by issue slots and latency, not by the FMA pipe, so halving the lane-parallel arithmetic instructions pays.
+// The (x,y) and (z,w) halves of a float4 that came from a 128-bit load are aligned pairs already (no moves).
+#define FT_X2_OP(name, op)                                                                                          \
+    __device__ __forceinline__ void name(float& d0, float& d1, float a0, float a1, float b0, float b1)              \
+    {                                                                                                               \
+        asm("{\n\t.reg .b64 ra, rb, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\t" op                    \
+            " rd, ra, rb;\n\tmov.b64 {%0, %1}, rd;\n\t}"                                                            \
+            : "=f"(d0), "=f"(d1) : "f"(a0), "f"(a1), "f"(b0), "f"(b1));                                             \
+    }
+FT_X2_OP(add2, "add.rn.f32x2")
+FT_X2_OP(sub2, "sub.rn.f32x2")
+FT_X2_OP(mul2, "mul.rn.f32x2")
+__device__ __forceinline__ void fma2(float& d0, float& d1, float a0, float a1, float b0, float b1, float c0, float c1)
+{
+    asm("{\n\t.reg .b64 ra, rb, rc, rd;\n\tmov.b64 ra, {%2, %3};\n\tmov.b64 rb, {%4, %5};\n\tmov.b64 rc, {%6, %7};\n\t"
+        "fma.rn.f32x2 rd, ra, rb, rc;\n\tmov.b64 {%0, %1}, rd;\n\t}"
+        : "=f"(d0), "=f"(d1) : "f"(a0), "f"(a1), "f"(b0), "f"(b1), "f"(c0), "f"(c1));
+}
+__device__ __forceinline__ float4 operator+(float4 a, float4 b) { float4 d; add2(d.x, d.y, a.x, a.y, b.x, b.y); add2(d.z, d.w, a.z, a.w, b.z, b.w); return d; }
+__device__ __forceinline__ float4 operator-(float4 a, float4 b) { float4 d; sub2(d.x, d.y, a.x, a.y, b.x, b.y); sub2(d.z, d.w, a.z, a.w, b.z, b.w); return d; }
+__device__ __forceinline__ float4 operator*(float4 a, float4 b) { float4 d; mul2(d.x, d.y, a.x, a.y, b.x, b.y); mul2(d.z, d.w, a.z, a.w, b.z, b.w); return d; }
+__device__ __forceinline__ float4 operator*(float a, float4 b) { float4 d; mul2(d.x, d.y, a, a, b.x, b.y); mul2(d.z, d.w, a, a, b.z, b.w); return d; }
 __device__ __forceinline__ float4 fma4(float4 a, float4 b, float4 c)
 {
-    return make_float4(fmaf(a.x, b.x, c.x), fmaf(a.y, b.y, c.y), fmaf(a.z, b.z, c.z), fmaf(a.w, b.w, c.w));
+    float4 d; fma2(d.x, d.y, a.x, a.y, b.x, b.y, c.x, c.y); fma2(d.z, d.w, a.z, a.w, b.z, b.w, c.z, c.w); return d;
 }
 __device__ __forceinline__ float4 fma4(float a, float4 b, float4 c)
 {
-    return make_float4(fmaf(a, b.x, c.x), fmaf(a, b.y, c.y), fmaf(a, b.z, c.z), fmaf(a, b.w, c.w));
+    float4 d; fma2(d.x, d.y, a, a, b.x, b.y, c.x, c.y); fma2(d.z, d.w, a, a, b.z, b.w, c.z, c.w); return d;
 }
+// lane-wise sum where one operand is not pair aligned (a quad shifted by one lane): scalar adds, no register moves
+__device__ __forceinline__ float4 adds(float4 a, float4 b) { return make_float4(a.x + b.x, a.y + b.y, a.z + b.z, a.w + b.w); }
 // the value one x to the right of each lane of `c`, `r0` being the element after c.w
 __device__ __forceinline__ float4 shl1(float4 c, float r0) { return make_float4(c.y, c.z, c.w, r0); }
 // 1/x by the special-function unit (MUFU.RCP, <= 1 ulp): 1/inf = 0 (fluid: mu = 0), 1/0 = inf
@@ -163,10 +191,7 @@ __device__ __forceinline__ float4 rcp4(float4 a) { return make_float4(rcpa(a.x),
 // Taps t0..t3 at consecutive samples: D+ at i uses (i-1, i, i+1, i+2) ; D- at i uses (i-2, i-1, i, i+1).
 #define FT_K 27.0f
 __device__ __forceinline__ float d1(float t0, float t1, float t2, float t3) { return fmaf(-FT_K, t2 - t1, t3 - t0); }
-__device__ __forceinline__ float4 d4(float4 t0, float4 t1, float4 t2, float4 t3)
-{
-    return make_float4(d1(t0.x, t1.x, t2.x, t3.x), d1(t0.y, t1.y, t2.y, t3.y), d1(t0.z, t1.z, t2.z, t3.z), d1(t0.w, t1.w, t2.w, t3.w));
-}
+__device__ __forceinline__ float4 d4(float4 t0, float4 t1, float4 t2, float4 t3) { return fma4(-FT_K, t2 - t1, t3 - t0); }
 // along x on a quad c = f[0..3]: l = (f[-2], f[-1]), r = (f[4], f[5])
 __device__ __forceinline__ float4 dpx(float2 l, float4 c, float2 r)   // D+ : result at i + 1/2
 {
@@ -190,17 +215,6 @@ __device__ __forceinline__ void ldg4_into(float4& v, const float* p, bool pred)
         "}"
         : "+f"(v.x), "+f"(v.y), "+f"(v.z), "+f"(v.w)
         : "l"(p), "r"((int)pred));
-}
-// L2 prefetch of the line(s) holding the quad at p (memory variables of the next plane: their loads then hit L2
-// instead of exposing a DRAM latency per stage)
-__device__ __forceinline__ void pf_l2(const float* p, bool pred)
-{
-    asm volatile(
-        "{\n\t"
-        ".reg .pred p;\n\t"
-        "setp.ne.b32 p, %1, 0;\n\t"
-        "@p prefetch.global.L2 [%0];\n\t"
-        "}" ::"l"(p), "r"((int)pred));
 }
 __device__ __forceinline__ void stg4(float* p, float4 v) { *reinterpret_cast<float4*>(p) = v; }
 
@@ -414,34 +428,47 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
     const int cx40 = x0 - 4 + PACT_HALO_X, cy40 = y0 - 4 + PACT_HALO_Y, cy36 = y0 - 2 + PACT_HALO_Y;
     const int cxm = x0 + PACT_HALO_X, cym = y0 + PACT_HALO_Y;
     const int cz0 = zb - 2 + PACT_HALO_Z;   // padded z of relative plane j = 0
+    // material-plane flags of this tile, relative plane j at mfl[j] (thread 0 only reads them)
+    const unsigned char* mfl = a.mflag ? a.mflag + ((size_t)wk.y * a.ntx + (wk.x & 0xffff)) * a.nzp + cz0 : nullptr;
+    auto mflag_at = [&](int j) -> unsigned { return mfl ? (unsigned)__ldg(mfl + j) : 0u; };
+    // padded z of the material plane to fetch for relative plane j, given its flag
+    auto mz = [&](int j, unsigned f) { return f ? a.mpal + (int)f - 1 : cz0 + j; };
+    // flags of the planes the next issues need, newest in the low byte: after the update in iteration `it`
+    // byte 0 = plane it + 3, ..., byte 3 = plane it, byte 4 = plane it - 1
+    unsigned long long fh = 0;
 
-    // E(j): s13, s23, rho, alpha of plane j -> slot j % 3
-    auto issueE = [&](int j, uint64_t* bar) {
+    // E(j): s13, s23, rho, alpha of plane j -> slot j % 3 ; f = material flag of plane j ; keep = the slot already
+    // holds this plane's rho and alpha (the plane three below came from the same palette plane): nothing to fetch
+    auto issueE = [&](int j, uint64_t* bar, unsigned f, bool keep) {
         const int s = j % 3;
         tma_plane(&tmS36, sm + FT_OFF_S13 + s * FT_UPL, bar, cx40, cy36, cz0 + j, S13);
         tma_plane(&tmS40, sm + FT_OFF_S23 + s * FT_BOX, bar, cx40, cy40, cz0 + j, S23);
-        tma_plane(&tmM37, sm + FT_OFF_RHO + s * FT_RPL, bar, cx40, cy36, cz0 + j, 2);
-        tma_plane(&tmM37, sm + FT_OFF_ALP + s * FT_RPL, bar, cx40, cy36, cz0 + j, 3);
+        if (!keep) {
+            tma_plane(&tmM37, sm + FT_OFF_RHO + s * FT_RPL, bar, cx40, cy36, mz(j, f), 2);
+            tma_plane(&tmM37, sm + FT_OFF_ALP + s * FT_RPL, bar, cx40, cy36, mz(j, f), 3);
+        }
     };
     // group c = what stage 1 of iteration c reads for the first time:
     //   s11, s22, s12 of plane c -> slot c & 1 ; E(c + 1) ; s33 of plane c + 2 -> slot c & 1 ; (c = 0: E(0) too)
-    auto issueG = [&](int c) {
+    auto issueG = [&](int c, unsigned fE1, unsigned fE0, bool keep) {     // flags of planes c + 1 and (c = 0 only) 0
         uint64_t* bar = &barG[c & 1];
-        const uint32_t eBytes = (FT_UPL + FT_BOX + 2 * FT_BW * FT_RH) * 4;     // s13, s23, rho, alpha
-        mbar_expect_tx(bar, (2 * FT_UPL + 2 * FT_BOX) * 4 + eBytes + (c == 0 ? eBytes : 0));
+        const uint32_t mBytes = 2 * FT_BW * FT_RH * 4;                        // rho, alpha
+        const uint32_t eBytes = (FT_UPL + FT_BOX) * 4 + mBytes;               // s13, s23, rho, alpha
+        mbar_expect_tx(bar, (2 * FT_UPL + 2 * FT_BOX) * 4 + eBytes - (keep ? mBytes : 0) + (c == 0 ? eBytes : 0));
         tma_plane(&tmS36, sm + FT_OFF_S11 + (c & 1) * FT_UPL, bar, cx40, cy36, cz0 + c, S11);
         tma_plane(&tmS40, sm + FT_OFF_S22 + (c & 1) * FT_BOX, bar, cx40, cy40, cz0 + c, S22);
         tma_plane(&tmS40, sm + FT_OFF_S12 + (c & 1) * FT_BOX, bar, cx40, cy40, cz0 + c, S12);
-        issueE(c + 1, bar);
+        issueE(c + 1, bar, fE1, keep);
         tma_plane(&tmS36, sm + FT_OFF_S33 + (c & 1) * FT_UPL, bar, cx40, cy36, cz0 + c + 2, S33);
-        if (c == 0) issueE(0, bar);
+        if (c == 0) issueE(0, bar, fE0, false);
     };
-    auto issueM = [&](int j) {
+    // flags of planes j (mu) and j - 1 (lambda) ; keep*: the slot holds the same palette plane already
+    auto issueM = [&](int j, unsigned fmu, unsigned flam, bool keep_mu, bool keep_lam) {
         uint64_t* bar = &barM[j % 3];
-        mbar_expect_tx(bar, (FT_MW * FT_MH + 3 * FT_LPL) * 4);
-        tma_plane(&tmM36, sm + FT_OFF_MU + (j % 3) * FT_MPL, bar, cxm, cym, cz0 + j, 1);
+        mbar_expect_tx(bar, ((keep_mu ? 0 : FT_MW * FT_MH) + (keep_lam ? 2 : 3) * FT_LPL) * 4);
+        if (!keep_mu) tma_plane(&tmM36, sm + FT_OFF_MU + (j % 3) * FT_MPL, bar, cxm, cym, mz(j, fmu), 1);
         // lambda of plane j - 1 (read by stage 2 of iteration j + 1, which waits on this barrier) -> slot (j - 1) & 1
-        tma_plane(&tmL, sm + FT_OFF_LAM + ((j + 1) & 1) * FT_LPL, bar, cxm, cym, cz0 + j - 1, 0);
+        if (!keep_lam) tma_plane(&tmL, sm + FT_OFF_LAM + ((j + 1) & 1) * FT_LPL, bar, cxm, cym, mz(j - 1, flam), 0);
         // and the old s11, s22 of that plane (the tile itself): they are the sigma(ks) that stage 2 adds to
         tma_plane(&tmS32, sm + FT_OFF_SO + (2 * ((j + 1) & 1) + 0) * FT_LPL, bar, cxm, cym, cz0 + j - 1, S11);
         tma_plane(&tmS32, sm + FT_OFF_SO + (2 * ((j + 1) & 1) + 1) * FT_LPL, bar, cxm, cym, cz0 + j - 1, S22);
@@ -456,7 +483,11 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
         tma_plane(&tmS36, sm + FT_OFF_UR + (2 * FT_RING + c % FT_RING) * FT_UPL, bar, cx40, cy36, cz0 + c, U3);
     };
 
-    if (tid == 0) { issueG(0); issueG(1); issueU(0); }
+    if (tid == 0) {
+        const unsigned f0 = mflag_at(0), f1 = mflag_at(1), f2 = mflag_at(2);
+        fh = (unsigned long long)f2 | ((unsigned long long)f1 << 8) | ((unsigned long long)f0 << 16) | ((unsigned long long)mflag_at(-1) << 24);
+        issueG(0, f1, f0, false); issueG(1, f2, 0u, false); issueU(0);
+    }
 
     // register windows along z (own column)
     float4 w13a, w13b, w13c;          // s13 at kk-2, kk-1, kk
@@ -493,6 +524,8 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
 
     for (int it = 0; it < itn; ++it) {
         const int kk = zb - 2 + it;
+        unsigned fnew = 0;      // thread 0: material flag of plane it + 3, fetched half an iteration before its use
+        if (tid == 0) fnew = mflag_at(it + 3);
         // forward C-PML: the nine phi of this thread's quad at plane kk, issued together ahead of the wait
         // (one exposed latency per stage instead of nine serialised ones)
         float4 pm[9];
@@ -607,7 +640,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                 }
                 const float4 rxp = shl1(r0, PR[4 * uq + 4]), axp = shl1(a0, PA[4 * uq + 4]);
                 mbar_wait(&barU[it & 1], (it >> 1) & 1);      // u_old(kk) has landed in the ring slot
-                n1 = fma4(fma4(mh, a0 + axp, one), *reinterpret_cast<const float4*>(R1), (kB * rcp4(r0 + rxp)) * (t1 + t2 + t3));
+                n1 = fma4(fma4(mh, adds(a0, axp), one), *reinterpret_cast<const float4*>(R1), (kB * rcp4(adds(r0, rxp))) * (t1 + t2 + t3));
             }
             {   // ---- u2 at (x, y+1/2, z): D-x s12, D+y s22, D-z s23
                 const float2 l = ld2s(P12, 4 * q - 2), rr = ld2s(P12, 4 * q + 4);
@@ -693,43 +726,25 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                 ldg4_into(e2[0], a.mvi[exa] + i2, se2); ldg4_into(e2[1], a.mvi[3 + exa] + i2, se2); ldg4_into(e2[2], a.mvi[6 + exa] + i2, se2);
             }
         }
-        // L2 prefetch of the memory variables the next iteration reads (own quad): stage-1 arrays at plane kk + 1,
-        // stage-2 arrays at plane ks + 1 ; along z the adjoint's taps reach two planes further
-        if (MODE != FM_PLAIN && pml && (bx || by || kk - 6 < a.P || kk + 6 >= a.nz - 1 - a.P)) {
-            const int S1 = MODE == FM_ADJ ? 9 : 0, S2 = 9 - S1, zq = MODE == FM_ADJ ? 2 : 0;
-            {
-                const int z1 = kk + 1;
-                const bool ok = pok && (unsigned)z1 < (unsigned)a.nz;
-                const bool ex = ok && colq >= 0, ey = ok && prow >= 0;
-                const int pzr = pok ? yzslab_row(z1 + zq, a.nz, a.P) : -1;
-                const bool ez = pzr >= 0;
-                const long long ix = ex ? idx_x(a, colq, y, z1) : 0, iy = ey ? idx_y(a, x, prow, z1) : 0, iz = ez ? idx_z(a, x, y, pzr) : 0;
-                pf_l2(a.mvi[S1 + 0] + ix, ex); pf_l2(a.mvi[S1 + 3] + ix, ex); pf_l2(a.mvi[S1 + 6] + ix, ex);
-                pf_l2(a.mvi[S1 + 1] + iy, ey); pf_l2(a.mvi[S1 + 4] + iy, ey); pf_l2(a.mvi[S1 + 7] + iy, ey);
-                pf_l2(a.mvi[S1 + 2] + iz, ez); pf_l2(a.mvi[S1 + 5] + iz, ez); pf_l2(a.mvi[S1 + 8] + iz, ez);
-            }
-            {
-                const int z2 = kk - 1;
-                const bool ok = inner && (unsigned)z2 < (unsigned)a.nz;
-                const bool ex = ok && colq >= 0, ey = ok && prow >= 0;
-                const int pzr = inner ? yzslab_row(z2 + zq, a.nz, a.P) : -1;
-                const bool ez = pzr >= 0;
-                const long long ix = ex ? idx_x(a, colq, y, z2) : 0, iy = ey ? idx_y(a, x, prow, z2) : 0, iz = ez ? idx_z(a, x, y, pzr) : 0;
-                pf_l2(a.mvi[S2 + 0] + ix, ex); pf_l2(a.mvi[S2 + 3] + ix, ex); pf_l2(a.mvi[S2 + 6] + ix, ex);
-                pf_l2(a.mvi[S2 + 1] + iy, ey); pf_l2(a.mvi[S2 + 4] + iy, ey); pf_l2(a.mvi[S2 + 7] + iy, ey);
-                pf_l2(a.mvi[S2 + 2] + iz, ez); pf_l2(a.mvi[S2 + 5] + iz, ez); pf_l2(a.mvi[S2 + 8] + iz, ez);
-            }
-        }
         if (pml && tid >= 360 && tid < 364) {   // z table ring: plane kk + 3 (first read after the barrier)
             const int t = tid - 360, z = kk + 3;
             sm[FT_OFF_ZT + t * FT_ZRING + (z & (FT_ZRING - 1))] = (unsigned)z < (unsigned)a.nz ? __ldg(a.tab[2][t] + z) : 0.0f;
         }
         __syncthreads();
         // every thread is past stage 1 of `it` and stage 2 of `it - 1`: refill the slots they freed
+        // thread 0: flags of planes it + 3 (E), it (mu), it - 1 (lambda) and of the planes that filled their slots last
+        unsigned fE = 0, fMu = 0, fLam = 0;
+        bool kE = false, kMu = false, kLam = false;
         if (tid == 0) {
+            fh = (fh << 8) | fnew;
+            fE = (unsigned)fh & 0xffu; fMu = (unsigned)(fh >> 24) & 0xffu; fLam = (unsigned)(fh >> 32) & 0xffu;
+            const unsigned fM3 = (unsigned)(fh >> 48) & 0xffu;             // plane it - 3: previous tenant of the mu and lambda slots
+            kE = fE != 0 && fE == fMu;                                     // rho, alpha slot (it + 3) % 3 holds plane it (>= 0)
+            kMu = it >= 3 && fMu != 0 && fMu == fM3;
+            kLam = it >= 2 && fLam != 0 && fLam == fM3;
             if (it + 1 < itn) issueU(it + 1);   // needed first ; slot of plane it - 4: its last cross-thread reads were in stage 2 of it - 2
-            if (it + 2 <= itn) issueM(it);
-            if (exa < 0 && it + 2 < itn) issueG(it + 2);   // exchange CTAs: after stage 2 (its slots are their scratch)
+            if (it + 2 <= itn) issueM(it, fMu, fLam, kMu, kLam);
+            if (exa < 0 && it + 2 < itn) issueG(it + 2, fE, 0u, kE);   // exchange CTAs: after stage 2 (its slots are their scratch)
         }
         if (it >= 1) mbar_wait(&barM[(it - 1) % 3], ((it - 1) / 3) & 1);
         // ------------------------------------------------------------------ stage 2: sigma(ks), ks = kk - 2
@@ -851,8 +866,9 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             const float4 i0 = ld4s(M0, mq), iy = ld4s(M0, mq + 9), iz = ld4s(M1, mq), iyz = ld4s(M1, mq + 9);
             const float4 ix = shl1(i0, M0[4 * mq + 4]), ixy = shl1(iy, M0[4 * mq + 40]), ixz = shl1(iz, M1[4 * mq + 4]);
             const float4 mn2 = kB * rcp4(i0);
-            const float4 mxy = kM * rcp4((i0 + ix) + (iy + ixy));
-            const float4 mxz = kM * rcp4((i0 + ix) + (iz + ixz));
+            const float4 i0x = adds(i0, ix);
+            const float4 mxy = kM * rcp4(i0x + adds(iy, ixy));
+            const float4 mxz = kM * rcp4(i0x + adds(iz, ixz));
             const float4 myz = kM * rcp4((i0 + iy) + (iz + iyz));
             const float4 lam = ld4s(sm + FT_OFF_LAM + (it & 1) * FT_LPL, (r - 2) * 8 + (qx - 1));   // lambda(ks), by TMA
             const float4 ldiv = (kL * lam) * (e11 + e22 + e33);
@@ -873,7 +889,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
         }
         if (exa >= 0) {   // every thread is done with the exchange planes: now the group that refills them may go
             __syncthreads();
-            if (tid == 0 && it + 2 < itn) issueG(it + 2);
+            if (tid == 0 && it + 2 < itn) issueG(it + 2, fE, 0u, kE);
         }
         u3m2 = u3m1; u1m1 = cc1; u2m1 = cc2; u3m1 = cc3;
         // slide the z windows

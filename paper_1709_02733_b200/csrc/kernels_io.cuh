@@ -64,6 +64,40 @@ __global__ void k_scale_materials(const float* __restrict__ lam, const float* __
     Aa[dst] = alpha ? (float)((double)alpha[src] * dt) : 0.0f;
 }
 
+// ---- pact_create: homogeneous material planes -------------------------
+// One block per (tile, padded plane): are the four scaled materials each one bit pattern over the tile's whole box
+// (x0-4 .. x0+35, y0-4 .. y0+35, clipped to the padded array) on that plane?  rec[(tile * nzp + zp)] = {homogeneous,
+// bits of Ll, Mi, Rr, Aa}.  The host turns the most frequent tuples into palette planes and per-plane flags.
+struct MatPlaneRec { unsigned int homog, v[4]; };
+__global__ void k_scan_material_planes(const float* __restrict__ mat /* start of the padded box of field 0 */, long long mbox,
+                                       int pitch, int py, int pz, int ntx, int nzp, MatPlaneRec* rec)
+{
+    const int tile = blockIdx.x, zp = blockIdx.y;
+    const int tx = tile % ntx, ty = tile / ntx;
+    MatPlaneRec r;
+    r.homog = 0; r.v[0] = r.v[1] = r.v[2] = r.v[3] = 0;
+    if (zp < pz) {
+        const int xa = tx * 32 - 4 + PACT_HALO_X, ya = ty * 32 - 4 + PACT_HALO_Y;
+        const int x0 = max(xa, 0), x1 = min(xa + 40, pitch), y0 = max(ya, 0), y1 = min(ya + 40, py);
+        const int w = x1 - x0, n = w * (y1 - y0);
+        bool same = true;
+        for (int k = 0; k < 4; ++k) {
+            const unsigned int* f = reinterpret_cast<const unsigned int*>(mat + (long long)k * mbox + (long long)zp * pitch * py);
+            const unsigned int first = f[(long long)y0 * pitch + x0];
+            r.v[k] = first;
+            for (int i = threadIdx.x; i < n; i += blockDim.x) same &= f[(long long)(y0 + i / w) * pitch + x0 + i % w] == first;
+        }
+        r.homog = __syncthreads_and(same) ? 1u : 0u;
+    }
+    if (threadIdx.x == 0) rec[(long long)tile * nzp + zp] = r;
+}
+
+__global__ void k_fill(float* p, unsigned int bits, long long n)
+{
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        p[i] = __uint_as_float(bits);
+}
+
 // ---- option "check_finite": flag <- 1 if any of the n values is a NaN or an Inf ------------------------
 __global__ void k_check_finite(const float* __restrict__ v, long long n, unsigned int* flag)
 {

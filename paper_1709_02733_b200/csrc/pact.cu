@@ -20,6 +20,7 @@
 #include "kernels_io.cuh"
 #include "kernels_plain.cuh"
 #include "kernels_fused.cuh"
+#include "kernels_pgd.cuh"
 
 
 // ------------------------------------------------------------------------------------------------
@@ -48,6 +49,11 @@ struct pact_ctx {
     int L;
     int pitch, py, pz;       // padded box extents
     long long box;           // elements of one padded field
+    long long mbox;          // elements of one padded material field: PACT_NPAL palette planes follow its pz planes
+    unsigned char* d_mflag;  // [tiles][nzp] material-plane flags of the fused path (kernels_fused.cuh)
+    int nzp;
+    double elided;           // fraction of (tile, plane) material boxes the fused path fetches from a palette plane
+    int elide;               // option "material_elision"
     DevGrid g;
     RcvTables rcv;
     IoArgs* d_io;
@@ -75,9 +81,11 @@ struct pact_ctx {
     unsigned int* d_queue;   // [2] ticket counter + exit counter of the persistent launch
     int split_launch;        // diagnostic option: slab bricks and interior bricks as two launches, timed apart
     float* mvbuf[2][18];     // fused memory variables, two sets (read / written alternate every step)
-    // host-buffer variants
+    // host-buffer variants and pact_pgd / pact_power_iteration (gradient and residual)
     float* d_vol;            // [N]
     float* d_dat;            // [nt][L]
+    double* d_partial;       // [PGD_MAXBLOCKS] block partial sums of the fp64 norms
+    double* d_norms;         // [PGD_MAXNORMS] norms left on the device by a pact_pgd / pact_power_iteration call
     // options
     int variant;             // 0 auto, 1 plain, 2 tiled
     int use_graph;           // -1 auto, 0 off, 1 on
@@ -177,6 +185,21 @@ extern "C" const char* pact_strerror(int code)
 extern "C" const char* pact_last_cuda_error(void) { return g_cuda_err; }
 
 extern "C" long long pact_device_bytes(const pact_ctx* c) { return c ? c->bytes : 0; }
+
+static int ensure_fused(pact_ctx* c);
+
+extern "C" int pact_get_info(pact_ctx* c, const char* key, double* value)
+{
+    if (!c || !key || !value) return PACT_EINVAL;
+    if (!strcmp(key, "elided_material_planes")) {
+        int rc = ensure_fused(c);
+        if (rc) return rc;
+        *value = c->elided;
+        return PACT_OK;
+    }
+    if (!strcmp(key, "num_sms")) { *value = c->num_sms; return PACT_OK; }
+    return PACT_EINVAL;
+}
 
 // ------------------------------------------------------------------------------------------------
 // pact_create
@@ -289,8 +312,9 @@ static int create_impl(pact_ctx* c, const pact_params* prm, const float* lam, co
 
     // ---- 4. scaled, padded material volumes
     float* mat = nullptr;
-    if ((rc = dev_alloc(c, (void**)&mat, (size_t)c->box * 4 * sizeof(float)))) return rc;
-    float* Ll = mat + org; float* Mi = Ll + c->box; float* Rr = Mi + c->box; float* Aa = Rr + c->box;
+    c->mbox = (long long)c->pitch * c->py * (c->pz + PACT_NPAL);
+    if ((rc = dev_alloc(c, (void**)&mat, (size_t)c->mbox * 4 * sizeof(float)))) return rc;
+    float* Ll = mat + org; float* Mi = Ll + c->mbox; float* Rr = Mi + c->mbox; float* Aa = Rr + c->mbox;
     {
         dim3 blk(128), grd((c->pitch + 127) / 128, c->py, c->pz);
         k_scale_materials<<<grd, blk, 0, c->stream>>>(lam, mu, rho, alpha, nx, ny, nz, g.sy, g.sz, c->pitch,
@@ -350,6 +374,7 @@ extern "C" int pact_create(pact_ctx** out, const pact_params* prm, const float* 
     c->variant = 0;
     c->use_graph = -1;
     c->split_launch = 1;
+    c->elide = 1;
     int rc = create_impl(c, prm, lam, mu, rho, alpha, rcv_xyz, L);
     if (rc != PACT_OK) { pact_destroy(c); return rc; }
     *out = c;
@@ -442,10 +467,12 @@ typedef CUresult (*encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_
                                     CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 // 4-D map [field][z][y][x] over `nf` padded fields starting at `base` (start of the padded box), box {bw, bh, 1, 1}
-static int make_map(pact_ctx* c, encode_tiled_fn enc, CUtensorMap* tm, const float* base, int nf, int bw, int bh)
+static int make_map(pact_ctx* c, encode_tiled_fn enc, CUtensorMap* tm, const float* base, int nf, int bw, int bh,
+                    int planes = 0, long long field_stride = 0)
 {
-    const cuuint64_t dims[4] = {(cuuint64_t)c->pitch, (cuuint64_t)c->py, (cuuint64_t)c->pz, (cuuint64_t)nf};
-    const cuuint64_t strides[3] = {(cuuint64_t)c->pitch * 4, (cuuint64_t)c->pitch * c->py * 4, (cuuint64_t)c->box * 4};
+    if (planes == 0) { planes = c->pz; field_stride = c->box; }
+    const cuuint64_t dims[4] = {(cuuint64_t)c->pitch, (cuuint64_t)c->py, (cuuint64_t)planes, (cuuint64_t)nf};
+    const cuuint64_t strides[3] = {(cuuint64_t)c->pitch * 4, (cuuint64_t)c->pitch * c->py * 4, (cuuint64_t)field_stride * 4};
     const cuuint32_t boxd[4] = {(cuuint32_t)bw, (cuuint32_t)bh, 1, 1};
     const cuuint32_t es[4] = {1, 1, 1, 1};
     // L2 promotion 64 B: box rows are 160 B starting 112 B into a 128-B line; with 128-B promotion every row pulls
@@ -456,6 +483,68 @@ static int make_map(pact_ctx* c, encode_tiled_fn enc, CUtensorMap* tm, const flo
         snprintf(g_cuda_err, sizeof(g_cuda_err), "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
         return PACT_ECUDA;
     }
+    return PACT_OK;
+}
+
+// Homogeneous material planes: flag every (tile, plane) whose material box is one 4-tuple, give the
+// PACT_NPAL most frequent tuples a palette plane each behind the material volumes, and let the fused kernel fetch
+// flagged planes from there.  Same bytes arrive in shared memory, so the result does not change by a bit; what
+// changes is that the palette planes live in L2 while the flagged planes are never read from HBM.
+static int scan_material_planes(pact_ctx* c)
+{
+    const DevGrid& g = c->g;
+    const int ntx = (g.nx + FT_TX - 1) / FT_TX, nty = (g.ny + FT_TY - 1) / FT_TY, tiles = ntx * nty;
+    c->nzp = c->pz + 8;
+    const long long nrec = (long long)tiles * c->nzp;
+    const long long org = (long long)PACT_HALO_Z * g.sz + (long long)PACT_HALO_Y * g.sy + PACT_HALO_X;
+    float* mat0 = const_cast<float*>(g.Ll) - org;
+    MatPlaneRec* d_rec = nullptr;
+    CK(cudaMalloc((void**)&d_rec, (size_t)nrec * sizeof(MatPlaneRec)));
+    k_scan_material_planes<<<dim3(tiles, c->nzp), 128, 0, c->stream>>>(mat0, c->mbox, c->pitch, c->py, c->pz, ntx, c->nzp, d_rec);
+    std::vector<MatPlaneRec> rec((size_t)nrec);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaMemcpyAsync(rec.data(), d_rec, (size_t)nrec * sizeof(MatPlaneRec), cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    cudaFree(d_rec);
+    if (e != cudaSuccess) return cuda_fail(e, "k_scan_material_planes", __LINE__);
+    // palette = the most frequent homogeneous tuples
+    struct Entry { unsigned int v[4]; long long n; };
+    std::vector<Entry> ent;
+    for (const MatPlaneRec& r : rec) {
+        if (!r.homog) continue;
+        size_t k = 0;
+        for (; k < ent.size(); ++k)
+            if (!memcmp(ent[k].v, r.v, sizeof(r.v))) break;
+        if (k == ent.size()) {
+            if (ent.size() >= 4096) continue;     // a medium with that many distinct homogeneous planes gains nothing here
+            Entry en; memcpy(en.v, r.v, sizeof(r.v)); en.n = 0;
+            ent.push_back(en);
+        }
+        ent[k].n++;
+    }
+    std::sort(ent.begin(), ent.end(), [](const Entry& a, const Entry& b) { return a.n > b.n; });
+    if (ent.size() > PACT_NPAL) ent.resize(PACT_NPAL);
+    std::vector<unsigned char> flag((size_t)nrec, 0);
+    long long hit = 0, planes = 0;
+    for (long long i = 0; i < nrec; ++i) {
+        if (i % c->nzp < c->pz) planes++;
+        if (!rec[(size_t)i].homog) continue;
+        for (size_t k = 0; k < ent.size(); ++k)
+            if (!memcmp(ent[k].v, rec[(size_t)i].v, sizeof(ent[k].v))) { flag[(size_t)i] = (unsigned char)(k + 1); hit++; break; }
+    }
+    c->elided = planes ? (double)hit / (double)planes : 0.0;
+    const long long plane = (long long)c->pitch * c->py;
+    for (size_t k = 0; k < ent.size(); ++k)
+        for (int f = 0; f < 4; ++f) {
+            k_fill<<<64, 256, 0, c->stream>>>(mat0 + (long long)f * c->mbox + (long long)(c->pz + (int)k) * plane, ent[k].v[f], plane);
+            CK(cudaGetLastError());
+        }
+    int rc = dev_alloc(c, (void**)&c->d_mflag, (size_t)nrec);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(c->d_mflag, flag.data(), (size_t)nrec, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaStreamSynchronize(c->stream));   // the vector is a temporary
+    c->fa.mflag = c->d_mflag;
+    c->fa.ntx = ntx; c->fa.nzp = c->nzp; c->fa.mpal = c->pz;
     return PACT_OK;
 }
 
@@ -517,13 +606,13 @@ static int ensure_fused(pact_ctx* c)
     if ((rc = make_map(c, enc, &c->tmS32[0], baseA, NFIELD, FT_TX, FT_TY))) return rc;
     if ((rc = make_map(c, enc, &c->tmS32[1], baseB, NFIELD, FT_TX, FT_TY))) return rc;
     if ((rc = make_map(c, enc, &c->tmS36[1], baseB, NFIELD, FT_BW, FT_UH))) return rc;
-    if ((rc = make_map(c, enc, &c->tmM37, baseM, 4, FT_BW, FT_RH))) return rc;
-    if ((rc = make_map(c, enc, &c->tmL, baseM, 4, FT_TX, FT_TY))) return rc;
-    if ((rc = make_map(c, enc, &c->tmM36, baseM, 4, FT_MW, FT_MH))) return rc;
+    if ((rc = make_map(c, enc, &c->tmM37, baseM, 4, FT_BW, FT_RH, c->pz + PACT_NPAL, c->mbox))) return rc;
+    if ((rc = make_map(c, enc, &c->tmL, baseM, 4, FT_TX, FT_TY, c->pz + PACT_NPAL, c->mbox))) return rc;
+    if ((rc = make_map(c, enc, &c->tmM36, baseM, 4, FT_MW, FT_MH, c->pz + PACT_NPAL, c->mbox))) return rc;
+    if ((rc = scan_material_planes(c))) return rc;
     CK(cudaFuncSetAttribute(k_step<FM_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
     CK(cudaFuncSetAttribute(k_step<FM_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
     CK(cudaFuncSetAttribute(k_step<FM_ADJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
-    fa.mat = g.Ll;
     c->work_zc = -1;
     c->work_cap = (long long)((g.nx + FT_TX - 1) / FT_TX) * ((g.ny + FT_TY - 1) / FT_TY) * (2 * g.nz + 2);   // worst case: one-plane chunks
     if ((rc = dev_alloc(c, (void**)&c->d_work, (size_t)c->work_cap * sizeof(int4)))) return rc;
@@ -611,6 +700,7 @@ static void fused_step(pact_ctx* c, Launcher& ln, int cur, float sgn, int kind)
     fa.in = gi.f[0]; fa.out = go.f[0];
     fa.sgn = sgn;
     fa.work = c->d_work;
+    fa.mflag = c->elide ? c->d_mflag : nullptr;
     for (int k = 0; k < 18; ++k) { fa.mvi[k] = c->mvbuf[cur][k]; fa.mvo[k] = c->mvbuf[1 - cur][k]; }
     cudaStream_t st = c->stream;
     auto launch = [&](int b0, int b1) {
@@ -814,6 +904,90 @@ extern "C" int pact_adjoint_host(pact_ctx* c, const float* data_host, float* ima
     return rc;
 }
 
+// ---- projected-gradient reconstruction ------------------------------
+#define PGD_MAXNORMS 4096
+static int ensure_pgd(pact_ctx* c)
+{
+    int rc = ensure_host_staging(c);
+    if (rc) return rc;
+    if (!c->d_partial && (rc = dev_alloc(c, (void**)&c->d_partial, PGD_MAXBLOCKS * sizeof(double)))) return rc;
+    if (!c->d_norms && (rc = dev_alloc(c, (void**)&c->d_norms, PGD_MAXNORMS * sizeof(double)))) return rc;
+    return PACT_OK;
+}
+
+static int pgd_blocks(const pact_ctx* c, long long n)
+{
+    const long long want = (n + PGD_BLOCK - 1) / PGD_BLOCK;
+    return (int)std::max(1ll, std::min(want, (long long)std::min(c->num_sms * 8, PGD_MAXBLOCKS)));
+}
+
+// p_{k+1} = P_+(p_k - s H^T (H p_k - d)), k = 0 .. iters-1.  Everything stays on the device; the two norms per
+// iteration are copied out once at the end (one synchronisation per call).
+extern "C" int pact_pgd(pact_ctx* c, float* p, const float* data, double step, int iters, int nonneg,
+                        double* resid_l2, double* update_l2)
+{
+    if (!c || !p || (!data && c->L > 0) || !(step > 0.0) || !std::isfinite(step) || iters < 0 || 2 * iters > PGD_MAXNORMS)
+        return PACT_EINVAL;
+    int rc = ensure_pgd(c);
+    if (rc) return rc;
+    const long long nd = (long long)c->prm.nt * c->L;
+    const int bd = pgd_blocks(c, nd), bn = pgd_blocks(c, c->N);
+    const int check = c->check_finite;
+    c->check_finite = 0;              // checked once, on the final iterate
+    for (int k = 0; k < iters && !rc; ++k) {
+        if ((rc = pact_forward(c, p, c->d_dat))) break;                       // H p_k
+        k_pgd_residual<<<bd, PGD_BLOCK, 0, c->stream>>>(c->d_dat, data, nd, c->d_partial);     // r = H p_k - d
+        k_pgd_finish<<<1, 32, 0, c->stream>>>(c->d_partial, bd, c->d_norms, 2 * k);
+        if ((rc = pact_adjoint(c, c->d_dat, c->d_vol))) break;                // g = H^T r
+        k_pgd_update<<<bn, PGD_BLOCK, 0, c->stream>>>(p, c->d_vol, (float)step, nonneg, c->N, c->d_partial);
+        k_pgd_finish<<<1, 32, 0, c->stream>>>(c->d_partial, bn, c->d_norms, 2 * k + 1);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) rc = cuda_fail(e, "pact_pgd kernels", __LINE__);
+    }
+    c->check_finite = check;
+    if (rc) return rc;
+    if (iters > 0 && (resid_l2 || update_l2)) {
+        std::vector<double> h((size_t)2 * iters);
+        CK(cudaMemcpyAsync(h.data(), c->d_norms, h.size() * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+        CK(cudaStreamSynchronize(c->stream));
+        for (int k = 0; k < iters; ++k) {
+            if (resid_l2) resid_l2[k] = h[(size_t)2 * k];
+            if (update_l2) update_l2[k] = h[(size_t)2 * k + 1];
+        }
+    }
+    return finite_check(c, p, c->N);
+}
+
+// ||H||^2 by power iteration on H^T H:  v <- H^T H v / ||H^T H v|| ; with ||v|| = 1 the norm before scaling tends to
+// the largest eigenvalue.  v is normalised first, so any non-zero start works (the caller supplies the seeded one).
+extern "C" int pact_power_iteration(pact_ctx* c, float* v, int iters, double* sigma2)
+{
+    if (!c || !v || iters < 1 || iters + 1 > PGD_MAXNORMS || !sigma2) return PACT_EINVAL;
+    int rc = ensure_pgd(c);
+    if (rc) return rc;
+    const int bn = pgd_blocks(c, c->N);
+    const int check = c->check_finite;
+    c->check_finite = 0;
+    for (int k = 0; k <= iters && !rc; ++k) {
+        k_pgd_norm2<<<bn, PGD_BLOCK, 0, c->stream>>>(v, c->N, c->d_partial);
+        k_pgd_finish<<<1, 32, 0, c->stream>>>(c->d_partial, bn, c->d_norms, k);          // k >= 1: ||H^T H v_{k-1}||
+        k_pgd_scale_by_inverse<<<bn, PGD_BLOCK, 0, c->stream>>>(v, c->N, c->d_norms, k);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) { rc = cuda_fail(e, "pact_power_iteration kernels", __LINE__); break; }
+        if (k == iters) break;
+        if ((rc = pact_forward(c, v, c->d_dat))) break;
+        if ((rc = pact_adjoint(c, c->d_dat, v))) break;
+    }
+    c->check_finite = check;
+    if (rc) return rc;
+    double h = 0.0;
+    CK(cudaMemcpyAsync(&h, c->d_norms + iters, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    *sigma2 = h;
+    if (!std::isfinite(h)) return PACT_ENUMERIC;
+    return PACT_OK;
+}
+
 // ---- options and timing -------------------------------------------------------------------------
 extern "C" int pact_set_option(pact_ctx* c, const char* key, long long value)
 {
@@ -827,6 +1001,7 @@ extern "C" int pact_set_option(pact_ctx* c, const char* key, long long value)
     }
     if (!strcmp(key, "zchunk")) { if (value < 0) return PACT_EINVAL; c->zchunk = (int)value; free_graphs(c); return PACT_OK; }
     if (!strcmp(key, "graph")) { c->use_graph = value < 0 ? -1 : (value != 0); return PACT_OK; }
+    if (!strcmp(key, "material_elision")) { c->elide = value != 0; free_graphs(c); return PACT_OK; }
     if (!strcmp(key, "split_launch")) { c->split_launch = value != 0; free_graphs(c); return PACT_OK; }
     return PACT_EINVAL;
 }

@@ -497,3 +497,65 @@ def test_long_run_at_the_stability_limit(torch_cuda, variant):
     d = ctx.forward(torch.from_numpy(pb.p0.astype(np.float32)).cuda()).cpu().numpy()
     ctx.close()
     assert np.abs(d[-200:]).max() <= 10 * np.abs(d[:200]).max()
+
+
+def test_material_elision_is_bit_exact(torch_cuda):
+    """Homogeneous (tile, plane) material boxes are fetched from a palette plane instead of their own plane
+    (DESIGN.md "Homogeneous material planes"): config 2 has two homogeneous media (water, brain) around a shell, so
+    most planes are elided -- and the operator must not change by a bit against the run that fetches every plane."""
+    torch = torch_cuda
+    prob = synth.make_config(2, nt=40)
+    y = np.random.default_rng(15).standard_normal((prob.prm.nt, prob.L)).astype(np.float32)
+    xd, yd = torch.from_numpy(prob.p0.astype(np.float32)).cuda(), torch.from_numpy(y).cuda()
+    out = []
+    for elide in (1, 0):
+        ctx = gpu_ops(torch, prob, variant=2, graph=0)
+        ctx.set_option("material_elision", elide)
+        if elide:
+            assert ctx.info("elided_material_planes") > 0.3
+        out.append((ctx.forward(xd).clone(), ctx.adjoint(yd).clone()))
+        ctx.close()
+    assert torch.equal(out[0][0], out[1][0]) and torch.equal(out[0][1], out[1][1])
+    # a random heterogeneous medium has nothing to elide
+    rp = synth.random_problem(nx=40, ny=36, nz=34, nt=4, npml=3, L=4, seed=16, lossy=True)
+    ctx = gpu_ops(torch, rp, variant=2)
+    assert ctx.info("elided_material_planes") == 0.0
+    ctx.close()
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_projected_gradient_matches_oracle(torch_cuda, variant):
+    """power-iteration step size and three projected-gradient iterations
+    p <- max(0, p - s H^T (H p - d)) through pact_power_iteration / pact_pgd against the same recursion on the fp64
+    oracle (oracle/pgd.py): step size to 1e-4, every iterate, residual norm and update norm to 1e-4."""
+    torch = torch_cuda
+    from oracle.oracle import Oracle
+    from oracle import pgd as opgd
+    prob = synth.random_problem(nx=44, ny=40, nz=36, nt=60, npml=5, L=24, seed=51, lossy=True)
+    rng = np.random.default_rng(51)
+    p_true = np.maximum(rng.standard_normal(prob.p0.shape), 0.0) * (rng.random(prob.p0.shape) < 0.05)
+    v0 = rng.standard_normal(prob.p0.shape).astype(np.float32)
+    o = Oracle.from_problem(prob)
+    d = o.forward(p_true.astype(np.float32).astype(np.float64))
+    d = (d + 0.01 * np.abs(d).max() * rng.standard_normal(d.shape)).astype(np.float32)
+    s2_o, _ = opgd.power_iteration(o, v0.astype(np.float64), iters=6)
+    its_o, res_o, upd_o = opgd.pgd(o, np.zeros(prob.p0.shape), d.astype(np.float64), 1.0 / s2_o, 3)
+    o.close()
+    ctx = gpu_ops(torch, prob, variant=variant)
+    ctx.set_option("check_finite", 1)
+    vd = torch.from_numpy(v0).cuda()
+    s2 = ctx.power_iteration(vd, iters=6)
+    assert abs(s2 - s2_o) <= 1e-4 * s2_o
+    assert abs(float(vd.double().norm()) - 1.0) <= 1e-5
+    dd = torch.from_numpy(d).cuda()
+    p = torch.zeros(ctx.shape, dtype=torch.float32, device="cuda")
+    for k in range(3):             # one iteration per call, so that every iterate can be compared
+        res, upd = ctx.pgd(p, dd, 1.0 / s2_o, 1)
+        assert_close(p.cpu().numpy(), its_o[k], f"iterate {k + 1}")
+        assert abs(res[0] - res_o[k]) <= 1e-4 * res_o[k] and abs(upd[0] - upd_o[k]) <= 1e-4 * upd_o[k]
+        assert float(p.min()) >= 0.0
+    # the same three iterations in one call give the same bits, and the residual decreases
+    p2 = torch.zeros_like(p)
+    res3, _ = ctx.pgd(p2, dd, 1.0 / s2_o, 3)
+    assert torch.equal(p, p2) and res3[0] > res3[1] > res3[2]
+    ctx.close()
