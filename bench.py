@@ -41,6 +41,9 @@ def parse_args():
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config (1-based); 4 is the headline")
     ap.add_argument("--nt", type=int, default=None, help="development only: truncate the number of samples")
     ap.add_argument("--variant", type=int, default=0, help="kernel variant (0 = library default)")
+    ap.add_argument("--pgd", action="store_true", help="SURVEY 8(f)-1: projected-gradient reconstruction (use with --config 5)")
+    ap.add_argument("--iters", type=int, default=10, help="--pgd: iterations")
+    ap.add_argument("--power-iters", type=int, default=8, help="--pgd: power iterations for the step size")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -228,10 +231,76 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def run_pgd(args):
+    """SURVEY 8(f)-1 / BASELINE config 5: d = H p_true + 1 % seeded Gaussian noise, step 1/||H||^2 from a power
+    iteration, then `--iters` iterations of p <- max(0, p - s H^T (H p - d)) through pact_pgd, one call per iteration
+    so that each is timed (CUDA events on the library's stream) and its image error is read.  One JSON line."""
+    import numpy as np
+    import torch
+    from paper_1709_02733_b200 import build, synth
+    from paper_1709_02733_b200.binding import Pact
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
+    torch.cuda.set_device(dev)
+    build.build()
+    prob = synth.make_config(args.config, nt=args.nt)
+    prm = prob.prm
+    ctx = Pact.from_problem(prob, device=dev)
+    ctx.set_option("variant", args.variant)
+    ctx.set_option("check_finite", 1)
+    rng = np.random.default_rng(170902733 + 100 * args.config)
+    p_true = torch.from_numpy(np.ascontiguousarray(prob.p0, dtype=np.float32)).to(dev)
+    d = ctx.forward(p_true)
+    noise = torch.from_numpy(rng.standard_normal((prm.nt, prob.L)).astype(np.float32)).to(dev)
+    d = d + 0.01 * float(d.abs().max()) * noise                      # SURVEY 8(d), config 5
+    del noise
+    v = torch.from_numpy(rng.standard_normal(ctx.shape).astype(np.float32)).to(dev)
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    e0, e1 = ev(), ev()
+    e0.record(ctx.stream)
+    sigma2 = ctx.power_iteration(v, args.power_iters)
+    e1.record(ctx.stream)
+    torch.cuda.synchronize(dev)
+    t_power = e0.elapsed_time(e1) * 1e-3
+    step = 1.0 / sigma2
+    p = torch.zeros(ctx.shape, dtype=torch.float32, device=dev)
+    nt2 = float(p_true.double().norm())
+    times, err, res, upd = [], [], [], []
+    clocks = ClockSampler(dev.index or 0)
+    clocks.start()
+    for k in range(args.iters):
+        a, b = ev(), ev()
+        a.record(ctx.stream)
+        r, u = ctx.pgd(p, d, step, 1)
+        b.record(ctx.stream)
+        torch.cuda.synchronize(dev)
+        times.append(a.elapsed_time(b) * 1e-3)
+        res.append(r[0]); upd.append(u[0])
+        err.append(float((p.double() - p_true.double()).norm()) / nt2)
+    clk = clocks.stop()
+    cells_iter = 2.0 * prm.N * (prm.nt - 1)
+    ts = sorted(times)
+    med = ts[len(ts) // 2]
+    line = {"metric": "seconds per projected-gradient iteration (one H and one H^T)", "value": med, "unit": "s",
+            "n_gpus": 1, "steps": args.iters, "warmup": 0, "ms_per_step": 1e3 * med, "higher_is_better": False,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": workload_name(prob, args) + "; d = H p_true + 1 % noise; p_0 = 0; step = 1/||H||^2",
+                       "power_iterations": args.power_iters, "elided_material_planes": ctx.info("elided_material_planes")},
+            "gcell_updates_per_s": cells_iter / med / 1e9, "sigma2": sigma2, "step": step, "power_iteration_s": t_power,
+            "seconds_per_iteration": times, "relative_image_error": err, "residual_l2": res, "update_l2": upd,
+            "data_l2": float(d.double().norm()), "clocks": clk,
+            "gpu_launches": int(args.iters * (2 * (2 * (prm.nt - 1) + prm.nt) + 8))}
+    print(json.dumps(line), flush=True)
+    ctx.close()
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+        return
+    if args.pgd:
+        run_pgd(args)
         return
     import numpy as np
     import torch

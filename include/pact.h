@@ -147,6 +147,9 @@ const char* pact_last_cuda_error(void);
  *              (interior) bricks as two launches on the context's stream, each timed on its own
  *              (PACT_K_*_SLAB / PACT_K_*_INTERIOR); 0: one persistent launch over the whole work list
  *              (PACT_K_*_FUSED).  Same bricks, same operator, same bits (measured within 2 % of each other).
+ *   "acoustic"  -1 (default): a medium with mu = 0 everywhere (the paper's H^dagger_{mu=0}) takes
+ *              the fused path's fluid-only kernels (one stress field + three velocities, 44 B per cell-step instead
+ *              of 88); 0: always the elastic kernels.  Same results to rounding (1-2 ulp).
  *   "material_elision"  1 (default): the fused path fetches (tile, plane) material boxes that are one constant
  *              4-tuple (water around a skull) from an L2-resident palette plane instead of HBM; 0: always the
  *              real plane.  Bit-identical results.
@@ -189,6 +192,8 @@ long long pact_device_bytes(const pact_ctx* ctx);
  *   "elided_material_planes"  fraction of the fused path's (32 x 32 tile, z plane) material boxes that are
  *                             homogeneous and served from a palette plane (builds the fused path's tables)
  *   "num_sms"                 multiprocessors of the context's device
+ *   "fluid"                   1 if mu = 0 everywhere in the medium
+ *   "acoustic_path"           1 if the next operator call runs the fluid-only kernels
  * Errors: PACT_EINVAL (NULL or unknown key), PACT_ENOMEM, PACT_ECUDA.
  */
 int pact_get_info(pact_ctx* ctx, const char* key, double* value);

@@ -11,7 +11,8 @@
 
 // ---- pact_create: scan the caller's volumes -----------------------------------------------------
 // flags bit 0: non-finite value ; bit 1: rho <= 0 ; bit 2: mu < 0 ; bit 3: lambda + 2 mu <= 0 ;
-// bit 4: alpha < 0 ; bit 5: 3 lambda + 2 mu <= 0 (legal, but the fused adjoint divides by it).  cmax2 = max (lambda + 2 mu)/rho as float bits (positive floats order as ints).
+// bit 4: alpha < 0 ; bit 5: 3 lambda + 2 mu <= 0 (legal, but the fused adjoint divides by it) ; bit 6: mu > 0 somewhere
+// (clear = a fluid everywhere: the acoustic specialisation applies).  cmax2 = max (lambda + 2 mu)/rho as float bits (positive floats order as ints).
 __global__ void k_scan_materials(const float* __restrict__ lam, const float* __restrict__ mu,
                                  const float* __restrict__ rho, const float* __restrict__ alpha,
                                  long long N, unsigned int* flags, unsigned int* cmax2_bits)
@@ -27,6 +28,7 @@ __global__ void k_scan_materials(const float* __restrict__ lam, const float* __r
         if (!(l + 2.0f * m > 0.0f)) f |= 8u;
         if (a < 0.0f) f |= 16u;
         if (!(3.0f * l + 2.0f * m > 0.0f)) f |= 32u;   // not an error: only rules out the scaled adjoint variables of the fused path
+        if (m > 0.0f) f |= 64u;
         if (r > 0.0f) c2 = fmaxf(c2, (l + 2.0f * m) / r);
     }
     for (int o = 16; o > 0; o >>= 1) {
@@ -153,7 +155,8 @@ struct RcvTables {
 };
 
 // Theta: one thread per receiver, fixed summation order c = 0..7
-__global__ void k_gather(const DevGrid g, const RcvTables r, const IoArgs* __restrict__ io, int m)
+// (fluid = 1: the acoustic path keeps the common normal stress in the S11 field only)
+__global__ void k_gather(const DevGrid g, const RcvTables r, const IoArgs* __restrict__ io, int m, int fluid = 0)
 {
     const int l = blockIdx.x * blockDim.x + threadIdx.x;
     if (l >= r.L) return;
@@ -164,7 +167,8 @@ __global__ void k_gather(const DevGrid g, const RcvTables r, const IoArgs* __res
 #pragma unroll
     for (int c = 0; c < 8; ++c) {
         const long long n = r.node8[8 * l + c];
-        acc = fmaf(r.w8[8 * l + c], s11[n] + s22[n] + s33[n], acc);
+        const float s = s11[n];
+        acc = fmaf(r.w8[8 * l + c], fluid ? s + s + s : s + s22[n] + s33[n], acc);
     }
     io->data_out[(long long)m * r.L + l] = -acc;
 }
@@ -186,7 +190,7 @@ __global__ void k_scatter(const DevGrid g, const RcvTables r, const IoArgs* __re
 // source that adds the same value v to the three normal components, C (v,v,v) = (3 Ll + 2 Ml) (v,v,v).
 __device__ __forceinline__ float bulk3(const DevGrid& g, long long n) { return 3.0f * g.Ll[n] + 2.0f / g.Mi[n]; }
 
-__global__ void k_scatter_scaled(const DevGrid g, const RcvTables r, const IoArgs* __restrict__ io, int m)
+__global__ void k_scatter_scaled(const DevGrid g, const RcvTables r, const IoArgs* __restrict__ io, int m, int fluid = 0)
 {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= r.nnodes) return;
@@ -195,17 +199,19 @@ __global__ void k_scatter_scaled(const DevGrid g, const RcvTables r, const IoArg
     for (int e = r.row_ptr[k]; e < r.row_ptr[k + 1]; ++e) acc = fmaf(r.tw[e], d[r.trcv[e]], acc);
     const long long n = r.tnode[k];
     acc *= bulk3(g, n);
-    g.f[S11][n] -= acc; g.f[S22][n] -= acc; g.f[S33][n] -= acc;
+    g.f[S11][n] -= acc;
+    if (!fluid) { g.f[S22][n] -= acc; g.f[S33][n] -= acc; }
 }
 
 // tau^T on the scaled variables: sigma_bar11+22+33 = (s11+s22+s33) / (3 Ll + 2 Ml)
-__global__ void k_image_scaled(const DevGrid g, const IoArgs* __restrict__ io)
+__global__ void k_image_scaled(const DevGrid g, const IoArgs* __restrict__ io, int fluid = 0)
 {
     const int x = blockIdx.x * blockDim.x + threadIdx.x;
     const int y = blockIdx.y * blockDim.y + threadIdx.y;
     const int z = blockIdx.z;
     if (x >= g.nx || y >= g.ny) return;
     const long long i = (long long)z * g.sz + (long long)y * g.sy + x;
+    const float s = g.f[S11][i];
     io->image[(long long)x + (long long)g.nx * ((long long)y + (long long)g.ny * z)] =
-        (g.f[S11][i] + g.f[S22][i] + g.f[S33][i]) / bulk3(g, i) * (-1.0f / 3.0f);
+        (fluid ? s + s + s : s + g.f[S22][i] + g.f[S33][i]) / bulk3(g, i) * (-1.0f / 3.0f);
 }

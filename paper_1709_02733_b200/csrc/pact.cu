@@ -21,6 +21,7 @@
 #include "kernels_plain.cuh"
 #include "kernels_fused.cuh"
 #include "kernels_pgd.cuh"
+#include "kernels_acoustic.cuh"
 
 
 // ------------------------------------------------------------------------------------------------
@@ -64,6 +65,8 @@ struct pact_ctx {
     long long state_bytes;
     float* scratch_base;     // adjoint scratch of the plain variant, allocated on first use
     // fused variant (kernels_fused.cuh): second state buffer, ping-pong memory variables, TMA maps
+    bool fluid;              // mu = 0 everywhere: the fused path runs its acoustic specialisation (option "acoustic")
+    int acoustic;            // option: -1 automatic (acoustic kernels when the medium is a fluid), 0 never
     bool bulk_positive;      // 3 lambda + 2 mu > 0 everywhere (the fused adjoint carries C sigma_bar and divides by it)
     bool fused_ready;
     DevGrid g2;              // view of state buffer B for the I/O kernels
@@ -187,6 +190,8 @@ extern "C" const char* pact_last_cuda_error(void) { return g_cuda_err; }
 extern "C" long long pact_device_bytes(const pact_ctx* c) { return c ? c->bytes : 0; }
 
 static int ensure_fused(pact_ctx* c);
+static int resolve_variant(const pact_ctx* c);
+static bool use_acoustic(const pact_ctx* c);
 
 extern "C" int pact_get_info(pact_ctx* c, const char* key, double* value)
 {
@@ -198,6 +203,8 @@ extern "C" int pact_get_info(pact_ctx* c, const char* key, double* value)
         return PACT_OK;
     }
     if (!strcmp(key, "num_sms")) { *value = c->num_sms; return PACT_OK; }
+    if (!strcmp(key, "fluid")) { *value = c->fluid ? 1.0 : 0.0; return PACT_OK; }
+    if (!strcmp(key, "acoustic_path")) { *value = (use_acoustic(c) && resolve_variant(c) == 2) ? 1.0 : 0.0; return PACT_OK; }
     return PACT_EINVAL;
 }
 
@@ -236,6 +243,7 @@ static int create_impl(pact_ctx* c, const pact_params* prm, const float* lam, co
     CK(cudaStreamSynchronize(c->stream));
     if (h_scan[0] & 31u) return PACT_EMATERIAL;
     c->bulk_positive = !(h_scan[0] & 32u);
+    c->fluid = !(h_scan[0] & 64u);
     float c2;
     memcpy(&c2, &h_scan[1], sizeof(float));
     const double cmax = std::sqrt((double)c2);
@@ -375,6 +383,7 @@ extern "C" int pact_create(pact_ctx** out, const pact_params* prm, const float* 
     c->use_graph = -1;
     c->split_launch = 1;
     c->elide = 1;
+    c->acoustic = -1;
     int rc = create_impl(c, prm, lam, mu, rho, alpha, rcv_xyz, L);
     if (rc != PACT_OK) { pact_destroy(c); return rc; }
     *out = c;
@@ -613,6 +622,9 @@ static int ensure_fused(pact_ctx* c)
     CK(cudaFuncSetAttribute(k_step<FM_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
     CK(cudaFuncSetAttribute(k_step<FM_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
     CK(cudaFuncSetAttribute(k_step<FM_ADJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
+    CK(cudaFuncSetAttribute(k_step_acoustic<FM_PLAIN>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
+    CK(cudaFuncSetAttribute(k_step_acoustic<FM_FWD>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
+    CK(cudaFuncSetAttribute(k_step_acoustic<FM_ADJ>, cudaFuncAttributeMaxDynamicSharedMemorySize, FT_SMEM_BYTES));
     c->work_zc = -1;
     c->work_cap = (long long)((g.nx + FT_TX - 1) / FT_TX) * ((g.ny + FT_TY - 1) / FT_TY) * (2 * g.nz + 2);   // worst case: one-plane chunks
     if ((rc = dev_alloc(c, (void**)&c->d_work, (size_t)c->work_cap * sizeof(int4)))) return rc;
@@ -690,6 +702,8 @@ static int build_work(pact_ctx* c)
     return PACT_OK;
 }
 
+static bool use_acoustic(const pact_ctx* c) { return c->fluid && c->acoustic != 0; }
+
 // one time step cur -> 1-cur ; sgn = +1: W' ; sgn = -1: W'^T on the scaled adjoint variables.  One persistent
 // launch (option "split_launch": the slab bricks and the interior bricks as two launches, each with its own events)
 static void fused_step(pact_ctx* c, Launcher& ln, int cur, float sgn, int kind)
@@ -707,7 +721,12 @@ static void fused_step(pact_ctx* c, Launcher& ln, int cur, float sgn, int kind)
         if (b1 <= b0) return;
         fa.work_begin = b0; fa.work_end = b1;
         const int grid = std::min(c->num_sms, b1 - b0);
-        if (fa.P == 0) k_step<FM_PLAIN><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fa);
+        if (use_acoustic(c)) {      // mu = 0 everywhere: one stress field, 44 B per cell-step (kernels_acoustic.cuh)
+            if (fa.P == 0) k_step_acoustic<FM_PLAIN><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmL, c->tmS32[cur], fa);
+            else if (sgn > 0.0f) k_step_acoustic<FM_FWD><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmL, c->tmS32[cur], fa);
+            else k_step_acoustic<FM_ADJ><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmL, c->tmS32[cur], fa);
+        }
+        else if (fa.P == 0) k_step<FM_PLAIN><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fa);
         else if (sgn > 0.0f) k_step<FM_FWD><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fa);
         else k_step<FM_ADJ><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fa);
     };
@@ -733,7 +752,8 @@ static int enqueue_forward_loop(pact_ctx* c, bool profile, int variant)
     for (int m = 0; m < nt; ++m) {
         ln.sample = profile && (m % every == every / 2);
         const DevGrid& gc = cur ? c->g2 : g;
-        if (c->L > 0) ln.run(PACT_K_RECV, [&] { k_gather<<<rgrd, rblk, 0, st>>>(gc, c->rcv, c->d_io, m); });
+        const int fl = variant == 2 && use_acoustic(c);
+        if (c->L > 0) ln.run(PACT_K_RECV, [&] { k_gather<<<rgrd, rblk, 0, st>>>(gc, c->rcv, c->d_io, m, fl); });
         if (m < nt - 1) {
             if (variant == 2) { fused_step(c, ln, cur, 1.0f, PACT_K_FWD_FUSED); cur ^= 1; }
             else forward_step(c, ln, variant);
@@ -761,7 +781,7 @@ static int enqueue_adjoint_loop(pact_ctx* c, bool profile, int variant)
         }
         const DevGrid& gc = cur ? c->g2 : g;
         if (c->L > 0) {
-            if (variant == 2) ln.run(PACT_K_RECV, [&] { k_scatter_scaled<<<rgrd, rblk, 0, st>>>(gc, c->rcv, c->d_io, m); });
+            if (variant == 2) ln.run(PACT_K_RECV, [&] { k_scatter_scaled<<<rgrd, rblk, 0, st>>>(gc, c->rcv, c->d_io, m, (int)use_acoustic(c)); });
             else ln.run(PACT_K_RECV, [&] { k_scatter<<<rgrd, rblk, 0, st>>>(gc, c->rcv, c->d_io, m); });
         }
     }
@@ -769,7 +789,7 @@ static int enqueue_adjoint_loop(pact_ctx* c, bool profile, int variant)
     {   // tau^T (Eq. 27c / 60c)
         const DevGrid& gc = cur ? c->g2 : g;
         dim3 blk(64, 4), grd((g.nx + 63) / 64, (g.ny + 3) / 4, g.nz);
-        if (variant == 2) ln.run(PACT_K_OTHER, [&] { k_image_scaled<<<grd, blk, 0, st>>>(gc, c->d_io); });
+        if (variant == 2) ln.run(PACT_K_OTHER, [&] { k_image_scaled<<<grd, blk, 0, st>>>(gc, c->d_io, (int)use_acoustic(c)); });
         else ln.run(PACT_K_OTHER, [&] { k_image<<<grd, blk, 0, st>>>(gc, c->d_io); });
     }
     return ln.err;
@@ -1001,6 +1021,7 @@ extern "C" int pact_set_option(pact_ctx* c, const char* key, long long value)
     }
     if (!strcmp(key, "zchunk")) { if (value < 0) return PACT_EINVAL; c->zchunk = (int)value; free_graphs(c); return PACT_OK; }
     if (!strcmp(key, "graph")) { c->use_graph = value < 0 ? -1 : (value != 0); return PACT_OK; }
+    if (!strcmp(key, "acoustic")) { c->acoustic = value < 0 ? -1 : (value != 0 ? -1 : 0); free_graphs(c); return PACT_OK; }
     if (!strcmp(key, "material_elision")) { c->elide = value != 0; free_graphs(c); return PACT_OK; }
     if (!strcmp(key, "split_launch")) { c->split_launch = value != 0; free_graphs(c); return PACT_OK; }
     return PACT_EINVAL;

@@ -559,3 +559,43 @@ def test_projected_gradient_matches_oracle(torch_cuda, variant):
     res3, _ = ctx.pgd(p2, dd, 1.0 / s2_o, 3)
     assert torch.equal(p, p2) and res3[0] > res3[1] > res3[2]
     ctx.close()
+
+
+ACOUSTIC_CASES = [
+    dict(nx=75, ny=70, nz=40, nt=30, npml=6, L=13, seed=61, lossy=True),      # 3 x 3 tiles, ragged, every brick touches a slab
+    dict(nx=130, ny=100, nz=64, nt=20, npml=5, L=9, seed=62, lossy=True),     # 5 x 4 tiles with C-PML-free bricks
+    dict(nx=40, ny=36, nz=33, nt=16, npml=0, L=5, seed=63, lossy=False),      # no C-PML, lossless
+]
+
+
+@pytest.mark.parametrize("case", ACOUSTIC_CASES, ids=lambda c: f"{c['nx']}x{c['ny']}x{c['nz']}_p{c['npml']}")
+def test_fluid_medium_takes_the_acoustic_kernels(torch_cuda, case):
+    """SURVEY 8(f)-2 (the paper's H^dagger_{mu=0}): a medium with mu = 0 everywhere runs the
+    fluid-only kernel pair of the fused path (one stress field + three velocities).  Parity and dot test against
+    the oracle run with mu = 0 (itself pinned against textbook acoustics), and agreement to rounding with the
+    elastic kernels on the same medium (option acoustic = 0)."""
+    torch = torch_cuda
+    prob = synth.random_problem(fluid_fraction=1.0, **case)
+    assert not prob.mu.any()
+    x, y = synth.random_vectors(prob, seed=case["seed"])
+    xd, yd = torch.from_numpy(x.astype(np.float32)).cuda(), torch.from_numpy(y.astype(np.float32)).cuda()
+    ctx = gpu_ops(torch, prob, variant=2, graph=0)
+    assert ctx.info("fluid") == 1.0 and ctx.info("acoustic_path") == 1.0
+    Hx, Hty = ctx.forward(xd).clone(), ctx.adjoint(yd).clone()
+    ctx.set_option("acoustic", 0)
+    assert ctx.info("acoustic_path") == 0.0
+    # the elastic kernels on the same medium: the same numbers up to the last bit of a few roundings (measured: 1-2 ulp)
+    for got, ref in ((Hx, ctx.forward(xd)), (Hty, ctx.adjoint(yd))):
+        assert float((got - ref).abs().max()) <= 2e-6 * float(ref.abs().max())
+    ctx.close()
+    Hx_o, Hty_o = oracle_pair(prob, x, y)
+    assert_close(Hx.cpu().numpy(), Hx_o)
+    assert_close(Hty.cpu().numpy(), Hty_o)
+    x32, y32 = x.astype(np.float32).astype(np.float64), y.astype(np.float32).astype(np.float64)
+    a, b = np.vdot(Hx.cpu().numpy().astype(np.float64), y32), np.vdot(x32, Hty.cpu().numpy().astype(np.float64))
+    assert abs(a - b) <= TOL_DOT * max(abs(a), abs(b))
+    # a medium with any solid cell keeps the elastic kernels
+    solid = synth.random_problem(nx=40, ny=36, nz=33, nt=4, npml=3, L=4, seed=64)
+    c2 = gpu_ops(torch, solid, variant=2)
+    assert c2.info("fluid") == 0.0 and c2.info("acoustic_path") == 0.0
+    c2.close()
