@@ -17,6 +17,25 @@
 #pragma once
 #include "kernels_fused.cuh"
 
+// Shared-memory map of the acoustic brick (floats; every plane 128-byte aligned).  With one stress field there is room
+// to spare, and it goes into latency: a u ring of AC_RING planes lets u_old(c) be requested three iterations ahead
+// (the elastic kernel can only ask half an iteration ahead, and waits for it), and the adjoint's exchange planes get
+// storage of their own instead of borrowing planes that a TMA refill is waiting for.
+#define AC_RING 6
+#define AC_OFF_S 0                                   // s(c), 40 x 40, 2 slots
+#define AC_OFF_W (AC_OFF_S + 2 * FT_BOX)             // s(c + 2), 40 x 36, 2 slots: feeds the z window
+#define AC_OFF_RHO (AC_OFF_W + 2 * FT_UPL)           // 3 slots
+#define AC_OFF_ALP (AC_OFF_RHO + 3 * FT_RPL)         // 3 slots
+#define AC_OFF_LAM (AC_OFF_ALP + 3 * FT_RPL)         // 2 slots
+#define AC_OFF_SO (AC_OFF_LAM + 2 * FT_LPL)          // old s of plane ks (tile only), 2 slots
+#define AC_OFF_UR (AC_OFF_SO + 2 * FT_LPL)           // u ring: [component][AC_RING] planes of 40 x 36
+#define AC_OFF_BARU (AC_OFF_UR + 3 * AC_RING * FT_UPL)   // 4 mbarriers (32 floats reserved)
+#define AC_OFF_SC1 (AC_OFF_BARU + 32)                // adjoint exchange plane of stage 1 (40 x 36)
+#define AC_OFF_SC2 (AC_OFF_SC1 + FT_UPL)             // adjoint exchange plane of stage 2
+static_assert(AC_OFF_SC2 + FT_BOX <= FT_OFF_END, "acoustic shared-memory map overlaps the barriers / tables");
+static_assert(AC_OFF_W % 32 == 0 && AC_OFF_RHO % 32 == 0 && AC_OFF_ALP % 32 == 0 && AC_OFF_LAM % 32 == 0 && AC_OFF_SO % 32 == 0 &&
+              AC_OFF_UR % 32 == 0 && AC_OFF_SC1 % 32 == 0, "TMA destinations are 128-byte aligned");
+
 template <int MODE>
 __device__ __forceinline__ void acoustic_brick(float* __restrict__ sm, const CUtensorMap& tmS40, const CUtensorMap& tmS36,
                                                const CUtensorMap& tmM37, const CUtensorMap& tmL, const CUtensorMap& tmS32,
@@ -25,7 +44,7 @@ __device__ __forceinline__ void acoustic_brick(float* __restrict__ sm, const CUt
     uint64_t* bars = reinterpret_cast<uint64_t*>(sm + FT_OFF_END);
     uint64_t* barG = bars;        // [2]  stress plane c, rho / alpha of plane c + 1, z-window plane c + 2
     uint64_t* barM = bars + 2;    // [3]  lambda and old stress of plane j - 1
-    uint64_t* barU = bars + 5;    // [2]  u_old of plane c
+    uint64_t* barU = reinterpret_cast<uint64_t*>(sm + AC_OFF_BARU);    // [4]  u_old of plane c, requested three iterations ahead
 
     const int tid = threadIdx.x;
     const int zb = wk.z, ze = wk.w;
@@ -74,6 +93,10 @@ __device__ __forceinline__ void acoustic_brick(float* __restrict__ sm, const CUt
             if (!first) mbar_inval(&bars[k]);
             mbar_init(&bars[k], 1);
         }
+        for (int k = 0; k < 4; ++k) {
+            if (!first) mbar_inval(&barU[k]);
+            mbar_init(&barU[k], 1);
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
@@ -91,36 +114,37 @@ __device__ __forceinline__ void acoustic_brick(float* __restrict__ sm, const CUt
     auto issueE = [&](int j, uint64_t* bar, unsigned f, bool keep) {
         if (keep) return;
         const int s = j % 3;
-        tma_plane(&tmM37, sm + FT_OFF_RHO + s * FT_RPL, bar, cx40, cy36, mz(j, f), 2);
-        tma_plane(&tmM37, sm + FT_OFF_ALP + s * FT_RPL, bar, cx40, cy36, mz(j, f), 3);
+        tma_plane(&tmM37, sm + AC_OFF_RHO + s * FT_RPL, bar, cx40, cy36, mz(j, f), 2);
+        tma_plane(&tmM37, sm + AC_OFF_ALP + s * FT_RPL, bar, cx40, cy36, mz(j, f), 3);
     };
     auto issueG = [&](int c, unsigned fE1, unsigned fE0, bool keep) {
         uint64_t* bar = &barG[c & 1];
         const uint32_t mBytes = 2 * FT_BW * FT_RH * 4;
         mbar_expect_tx(bar, (FT_BOX + FT_UPL) * 4 + (keep ? 0 : mBytes) + (c == 0 ? mBytes : 0));
-        tma_plane(&tmS40, sm + FT_OFF_S22 + (c & 1) * FT_BOX, bar, cx40, cy40, cz0 + c, S11);          // s(c), 40 x 40
+        tma_plane(&tmS40, sm + AC_OFF_S + (c & 1) * FT_BOX, bar, cx40, cy40, cz0 + c, S11);          // s(c), 40 x 40
         issueE(c + 1, bar, fE1, keep);
-        tma_plane(&tmS36, sm + FT_OFF_S33 + (c & 1) * FT_UPL, bar, cx40, cy36, cz0 + c + 2, S11);      // s(c + 2): z window
+        tma_plane(&tmS36, sm + AC_OFF_W + (c & 1) * FT_UPL, bar, cx40, cy36, cz0 + c + 2, S11);      // s(c + 2): z window
         if (c == 0) issueE(0, bar, fE0, false);
     };
     auto issueM = [&](int j, unsigned flam, bool keep_lam) {      // lambda and old s of plane j - 1 -> slot (j - 1) & 1
         uint64_t* bar = &barM[j % 3];
         mbar_expect_tx(bar, (keep_lam ? 1 : 2) * FT_LPL * 4);
-        if (!keep_lam) tma_plane(&tmL, sm + FT_OFF_LAM + ((j + 1) & 1) * FT_LPL, bar, cxm, cym, mz(j - 1, flam), 0);
-        tma_plane(&tmS32, sm + FT_OFF_SO + (2 * ((j + 1) & 1)) * FT_LPL, bar, cxm, cym, cz0 + j - 1, S11);
+        if (!keep_lam) tma_plane(&tmL, sm + AC_OFF_LAM + ((j + 1) & 1) * FT_LPL, bar, cxm, cym, mz(j - 1, flam), 0);
+        tma_plane(&tmS32, sm + AC_OFF_SO + ((j + 1) & 1) * FT_LPL, bar, cxm, cym, cz0 + j - 1, S11);
     };
     auto issueU = [&](int c) {
-        uint64_t* bar = &barU[c & 1];
+        uint64_t* bar = &barU[c & 3];
         mbar_expect_tx(bar, 3 * FT_UPL * 4);
-        tma_plane(&tmS36, sm + FT_OFF_UR + (0 * FT_RING + c % FT_RING) * FT_UPL, bar, cx40, cy36, cz0 + c, U1);
-        tma_plane(&tmS36, sm + FT_OFF_UR + (1 * FT_RING + c % FT_RING) * FT_UPL, bar, cx40, cy36, cz0 + c, U2);
-        tma_plane(&tmS36, sm + FT_OFF_UR + (2 * FT_RING + c % FT_RING) * FT_UPL, bar, cx40, cy36, cz0 + c, U3);
+        tma_plane(&tmS36, sm + AC_OFF_UR + (0 * AC_RING + c % AC_RING) * FT_UPL, bar, cx40, cy36, cz0 + c, U1);
+        tma_plane(&tmS36, sm + AC_OFF_UR + (1 * AC_RING + c % AC_RING) * FT_UPL, bar, cx40, cy36, cz0 + c, U2);
+        tma_plane(&tmS36, sm + AC_OFF_UR + (2 * AC_RING + c % AC_RING) * FT_UPL, bar, cx40, cy36, cz0 + c, U3);
     };
 
     if (tid == 0) {
         const unsigned f0 = mflag_at(0), f1 = mflag_at(1), f2 = mflag_at(2);
         fh = (unsigned long long)f2 | ((unsigned long long)f1 << 8) | ((unsigned long long)f0 << 16) | ((unsigned long long)mflag_at(-1) << 24);
-        issueG(0, f1, f0, false); issueG(1, f2, 0u, false); issueU(0);
+        issueG(0, f1, f0, false); issueG(1, f2, 0u, false);
+        for (int c = 0; c < 3 && c < itn; ++c) issueU(c);
     }
 
     // z window of s (own column): planes kk-2 .. kk+1 ; stage 2's oldest u3 taps
@@ -136,8 +160,8 @@ __device__ __forceinline__ void acoustic_brick(float* __restrict__ sm, const CUt
     }
 
     const float kB = 2.0f * a.sgn * PACT_C2, kL = a.sgn * PACT_C2;
-    const float* Rbase = sm + FT_OFF_RHO;
-    const float* Abase = sm + FT_OFF_ALP;
+    const float* Rbase = sm + AC_OFF_RHO;
+    const float* Abase = sm + AC_OFF_ALP;
     const float* xt0 = sm + FT_OFF_XT + 8 - x0;
     const float* yt0 = sm + FT_OFF_YT + 8 - y0;
     const float* zt0 = sm + FT_OFF_ZT;
@@ -173,9 +197,9 @@ __device__ __forceinline__ void acoustic_brick(float* __restrict__ sm, const CUt
         const int s3 = it % 3, s3n = (it + 1) % 3;
         float4 f33 = z4;
         const bool zin = (unsigned)kk < (unsigned)a.nz;
-        const float* PS = sm + FT_OFF_S22 + (it & 1) * FT_BOX;                        // s(kk), 40 x 40
+        const float* PS = sm + AC_OFF_S + (it & 1) * FT_BOX;                          // s(kk), 40 x 40
         // ------------------------------------------------------------------ stage 1: u(kk)
-        float* const SC1 = sm + FT_OFF_UR + ((it + 1) % FT_RING) * FT_UPL + (exa == 1 ? FT_RING * FT_UPL : 0);
+        float* const SC1 = sm + AC_OFF_SC1;
         if (exa >= 0) {
             if (act1) {
                 float4 X = z4;
@@ -186,7 +210,6 @@ __device__ __forceinline__ void acoustic_brick(float* __restrict__ sm, const CUt
                     else X = adj_own_x(e1, a.mvo[13], ie1, se1, f4(YT(T_A_INT)[y]), f4(YT(T_B_INT)[y]), os, wr);
                 }
                 *reinterpret_cast<float4*>(SC1 + 4 * uq) = X;
-                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             }
             __syncthreads();
         }
@@ -194,7 +217,7 @@ __device__ __forceinline__ void acoustic_brick(float* __restrict__ sm, const CUt
         if (act1) {
             const float* PR = Rbase + s3 * FT_RPL;
             const float* PA = Abase + s3 * FT_RPL;
-            f33 = ld4s(sm + FT_OFF_S33 + (it & 1) * FT_UPL, uq);   // plane kk+2
+            f33 = ld4s(sm + AC_OFF_W + (it & 1) * FT_UPL, uq);   // plane kk+2
             const bool wr1 = inner && kk >= zb && kk < ze;
             const int pz = (pml && zin) ? yzslab_row(kk, a.nz, a.P) : -1;
             const bool bz = pml && (kk - 2 < a.P || kk + 2 >= a.nz - 1 - a.P);
@@ -204,17 +227,17 @@ __device__ __forceinline__ void acoustic_brick(float* __restrict__ sm, const CUt
             const float4 one = f4(1.0f), mh = f4(-0.5f);
             const float4 cs = ld4s(PS, q);
             float4 n1, n2, n3;
-            const int sl = it % FT_RING;
-            float* const R1 = sm + FT_OFF_UR + (0 * FT_RING + sl) * FT_UPL + 4 * uq;
-            float* const R2 = sm + FT_OFF_UR + (1 * FT_RING + sl) * FT_UPL + 4 * uq;
-            float* const R3 = sm + FT_OFF_UR + (2 * FT_RING + sl) * FT_UPL + 4 * uq;
+            const int sl = it % AC_RING;
+            float* const R1 = sm + AC_OFF_UR + (0 * AC_RING + sl) * FT_UPL + 4 * uq;
+            float* const R2 = sm + AC_OFF_UR + (1 * AC_RING + sl) * FT_UPL + 4 * uq;
+            float* const R3 = sm + AC_OFF_UR + (2 * AC_RING + sl) * FT_UPL + 4 * uq;
             {   // ---- u1 at (x+1/2, y, z): D+x s
                 float4 t1 = dpx(ld2s(PS, 4 * q - 2), cs, ld2s(PS, 4 * q + 4));
                 if (MODE == FM_FWD && pml1 && colq >= 0)
                     t1 = pml_fwd_m(pm0, a.mvo[0], idx_x(a, colq, y, kk), tab4(XT(T_A_HALF), x), tab4(XT(T_B_HALF), x), t1, wr1);
                 if (MODE == FM_ADJ && pml1 && exa == 0) t1 = t1 + dpx(ld2s(SC1, 4 * uq - 2), ld4s(SC1, uq), ld2s(SC1, 4 * uq + 4));
                 const float4 rxp = shl1(r0, PR[4 * uq + 4]), axp = shl1(a0, PA[4 * uq + 4]);
-                mbar_wait(&barU[it & 1], (it >> 1) & 1);
+                mbar_wait(&barU[it & 3], (it >> 2) & 1);
                 n1 = fma4(fma4(mh, adds(a0, axp), one), *reinterpret_cast<const float4*>(R1), (kB * rcp4(adds(r0, rxp))) * t1);
             }
             {   // ---- u2 at (x, y+1/2, z): D+y s
@@ -289,37 +312,37 @@ __device__ __forceinline__ void acoustic_brick(float* __restrict__ sm, const CUt
             const unsigned fIt = (unsigned)(fh >> 24) & 0xffu, fM3 = (unsigned)(fh >> 48) & 0xffu;
             kE = fE != 0 && fE == fIt;
             kLam = it >= 2 && fLam != 0 && fLam == fM3;
-            if (it + 1 < itn) issueU(it + 1);
+            // ring slot of plane it + 3 held plane it - 3, last read in stage 2 of iteration it - 1: free since this barrier
+            if (it + 3 < itn) issueU(it + 3);
             if (it + 2 <= itn) issueM(it, fLam, kLam);
-            if (exa < 0 && it + 2 < itn) issueG(it + 2, fE, 0u, kE);
+            if (it + 2 < itn) issueG(it + 2, fE, 0u, kE);
         }
         if (it >= 1) mbar_wait(&barM[(it - 1) % 3], ((it - 1) / 3) & 1);
         // ------------------------------------------------------------------ stage 2: s(ks), ks = kk - 2
         const int ks = kk - 2;
         float4 cc3 = z4;
-        if (inner && it >= 2) cc3 = ld4s(sm + FT_OFF_UR + 2 * FT_RING * FT_UPL + ((it + 2) % FT_RING) * FT_UPL, uq);
-        float* const SC2 = sm + FT_OFF_S22 + (it & 1) * FT_BOX;       // the stress plane stage 1 has finished with
+        if (inner && it >= 2) cc3 = ld4s(sm + AC_OFF_UR + 2 * AC_RING * FT_UPL + ((it + AC_RING - 2) % AC_RING) * FT_UPL, uq);
+        float* const SC2 = sm + AC_OFF_SC2;
         if (exa >= 0) {
             if (act1 && it >= 4) {
                 float4 Y = z4;
                 if (pok && (unsigned)ks < (unsigned)a.nz) {
-                    const int pc = ((it + 2) % FT_RING) * FT_UPL;
+                    const int pc = ((it + AC_RING - 2) % AC_RING) * FT_UPL;
                     if (exa == 0) Y = adj_own_x(e2, a.mvo[0], i2, se2, tab4(XT(T_A_HALF), x), tab4(XT(T_B_HALF), x),
-                                                ld4s(sm + FT_OFF_UR + 0 * FT_RING * FT_UPL + pc, uq), inner);
+                                                ld4s(sm + AC_OFF_UR + 0 * AC_RING * FT_UPL + pc, uq), inner);
                     else Y = adj_own_x(e2, a.mvo[4], i2, se2, f4(YT(T_A_HALF)[y]), f4(YT(T_B_HALF)[y]),
-                                       ld4s(sm + FT_OFF_UR + 1 * FT_RING * FT_UPL + pc, uq), inner);
+                                       ld4s(sm + AC_OFF_UR + 1 * AC_RING * FT_UPL + pc, uq), inner);
                 }
                 *reinterpret_cast<float4*>(SC2 + 4 * uq) = Y;
-                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             }
             __syncthreads();
         }
         if (inner && it >= 4) {
             const int j = it - 2;
-            const float* U1p = sm + FT_OFF_UR + 0 * FT_RING * FT_UPL;
-            const float* U2p = sm + FT_OFF_UR + 1 * FT_RING * FT_UPL;
-            const float* U3p = sm + FT_OFF_UR + 2 * FT_RING * FT_UPL;
-            const int p0 = (j % FT_RING) * FT_UPL, pp1 = ((j + 1) % FT_RING) * FT_UPL;
+            const float* U1p = sm + AC_OFF_UR + 0 * AC_RING * FT_UPL;
+            const float* U2p = sm + AC_OFF_UR + 1 * AC_RING * FT_UPL;
+            const float* U3p = sm + AC_OFF_UR + 2 * AC_RING * FT_UPL;
+            const int p0 = (j % AC_RING) * FT_UPL, pp1 = ((j + 1) % AC_RING) * FT_UPL;
             const int pz = pml ? yzslab_row(ks, a.nz, a.P) : -1;
             const bool bz = pml && (ks - 2 < a.P || ks + 2 >= a.nz - 1 - a.P);
             const bool pml2 = bx || by || bz;
@@ -348,14 +371,10 @@ __device__ __forceinline__ void acoustic_brick(float* __restrict__ sm, const CUt
                 if (MODE == FM_ADJ && pml2 && bz)
                     e33 = e33 + adj_z(a, a.mvi[8], a.mvo[8], ZT(T_A_HALF), ZT(T_B_HALF), x, y, ks - 2, 2, u3m2, u3m1, cc3, zd, true);
             }
-            const float4 lam = ld4s(sm + FT_OFF_LAM + (it & 1) * FT_LPL, lq);
+            const float4 lam = ld4s(sm + AC_OFF_LAM + (it & 1) * FT_LPL, lq);
             const float4 ldiv = (kL * lam) * (e11 + e22 + e33);
-            const float4 ns = ld4s(sm + FT_OFF_SO + (2 * (it & 1)) * FT_LPL, lq) + ldiv;
+            const float4 ns = ld4s(sm + AC_OFF_SO + (it & 1) * FT_LPL, lq) + ldiv;
             store_quad(a.out + S11 * box + (long long)ks * a.sz + gxy, ns, x, a.nx);
-        }
-        if (exa >= 0) {
-            __syncthreads();
-            if (tid == 0 && it + 2 < itn) issueG(it + 2, fE, 0u, kE);
         }
         u3m2 = u3m1; u3m1 = cc3;
         w33a = w33b; w33b = w33c; w33c = w33d; w33d = f33;
