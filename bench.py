@@ -41,6 +41,8 @@ def parse_args():
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config (1-based); 4 is the headline")
     ap.add_argument("--nt", type=int, default=None, help="development only: truncate the number of samples")
     ap.add_argument("--variant", type=int, default=0, help="kernel variant (0 = library default)")
+    ap.add_argument("--acoustic", action="store_true",
+                    help="SURVEY 8(f)-2: the config's medium with mu = 0 (H^dagger_{mu=0}, PAPER.md:299): fluid-only kernels, 44 B per cell-step")
     ap.add_argument("--pgd", action="store_true", help="SURVEY 8(f)-1: projected-gradient reconstruction (use with --config 5)")
     ap.add_argument("--iters", type=int, default=10, help="--pgd: iterations")
     ap.add_argument("--power-iters", type=int, default=8, help="--pgd: power iterations for the step size")
@@ -53,9 +55,23 @@ def parse_args():
 def workload_name(prob, args):
     p = prob.prm
     s = f"BASELINE config {args.config}: {p.nx}x{p.ny}x{p.nz}, nt={p.nt}, L={prob.L}, npml={p.npml}"
+    if getattr(args, "acoustic", False):
+        s += "; shear modulus set to zero (the paper's H_mu=0: fluid-only kernels)"
     if args.nt is not None:
         s += " (nt truncated: development run, not the headline)"
     return s
+
+
+def make_problem(args):
+    from paper_1709_02733_b200 import synth
+    prob = synth.make_config(args.config, nt=args.nt)
+    return synth.fluid_version(prob) if args.acoustic else prob
+
+
+def bytes_per_cell_step(args):
+    """Algorithmic bytes per cell per time step (DESIGN.md): elastic 9 state fields R+W + 4 materials R = 88;
+    fluid-only 4 state fields R+W + 3 materials R = 44."""
+    return 44.0 if args.acoustic else B_ALG
 
 
 def cpu_sample(prob):
@@ -101,7 +117,7 @@ def run_reference(args):
     if rank != 0:
         return
     from paper_1709_02733_b200 import synth
-    prob = synth.make_config(args.config, nt=args.nt)
+    prob = make_problem(args)
     sub, what = cpu_sample(prob)
     for _ in range(max(args.warmup, 0) and 1):
         time_oracle(sub)
@@ -243,7 +259,7 @@ def run_pgd(args):
     dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
     torch.cuda.set_device(dev)
     build.build()
-    prob = synth.make_config(args.config, nt=args.nt)
+    prob = make_problem(args)
     prm = prob.prm
     ctx = Pact.from_problem(prob, device=dev)
     ctx.set_option("variant", args.variant)
@@ -318,7 +334,7 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
     build.build()
 
-    prob = synth.make_config(args.config, nt=args.nt)     # every rank: an independent replica
+    prob = make_problem(args)                             # every rank: an independent replica
     prm = prob.prm
     ctx = Pact.from_problem(prob, device=dev)
     ctx.set_option("variant", args.variant)
@@ -377,19 +393,29 @@ def main():
     # device time of one time step's kernels (all launches of the step, in the mix they ran)
     step_kinds_f = ("fwd_vel", "fwd_str", "fwd_fused", "fwd_slab", "fwd_interior")
     step_kinds_a = ("adj_a", "adj_b", "adj_fused", "adj_slab", "adj_interior")
-    t_fwd = sum(k_f[k] * n_f[k] for k in step_kinds_f) / max(prm.nt - 1, 1)
-    t_adj = sum(k_a[k] * n_a[k] for k in step_kinds_a) / max(prm.nt - 1, 1)
+    # sampled launches (CUDA events around every ~80th launch): a cross-check and the slab / interior split
+    ts_fwd = sum(k_f[k] * n_f[k] for k in step_kinds_f) / max(prm.nt - 1, 1)
+    ts_adj = sum(k_a[k] * n_a[k] for k in step_kinds_a) / max(prm.nt - 1, 1)
+    # basis of the roofline: the whole time loop of the last timed forward / adjoint call (events on the library's
+    # stream around the loop) divided by its nt - 1 steps.  It contains the receiver kernels (< 0.4 % of a step) and
+    # no event overhead; the sampled per-launch times read a few per cent higher because every sampled launch
+    # carries two event records and the launch gap.
+    t_fwd = loop_f / max(prm.nt - 1, 1)
+    t_adj = loop_a / max(prm.nt - 1, 1)
     peak, peak_src = peaks()
-    pml_extra = 48.0 * 3 * 2 * prm.npml / prm.nx if prm.npml else 0.0
+    pml_extra = (16.0 if args.acoustic else 48.0) * 3 * 2 * prm.npml / prm.nx if prm.npml else 0.0
     roof = None
     if t_fwd > 0 and t_adj > 0:
-        ach = 2 * B_ALG * prm.N / ((t_fwd + t_adj) * 1e-3) / 1e9
+        B = bytes_per_cell_step(args)
+        ach = 2 * B * prm.N / ((t_fwd + t_adj) * 1e-3) / 1e9
         roof = {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
                 "peak_source": peak_src, "kernel": "step kernels of one forward + one adjoint time step",
-                "bytes_per_cell_step": B_ALG, "pml_bytes_per_cell_step_not_credited": pml_extra,
+                "basis": "time loop of the last timed forward / adjoint call / (nt - 1) steps, CUDA events on the library's stream",
+                "sampled_forward_step_ms": ts_fwd, "sampled_adjoint_step_ms": ts_adj,
+                "bytes_per_cell_step": B, "pml_bytes_per_cell_step_not_credited": pml_extra,
                 "forward_step_ms": t_fwd, "adjoint_step_ms": t_adj,
-                "forward_frac": B_ALG * prm.N / (t_fwd * 1e-3) / 1e9 / peak,
-                "adjoint_frac": B_ALG * prm.N / (t_adj * 1e-3) / 1e9 / peak,
+                "forward_frac": B * prm.N / (t_fwd * 1e-3) / 1e9 / peak,
+                "adjoint_frac": B * prm.N / (t_adj * 1e-3) / 1e9 / peak,
                 "forward_loop_ms": loop_f, "adjoint_loop_ms": loop_a,
                 "kernel_ms": {"forward": {k: v for k, v in k_f.items() if v}, "adjoint": {k: v for k, v in k_a.items() if v}}}
         t, src = committed_traffic(args.config)
@@ -397,7 +423,7 @@ def main():
         if t:
             # per launch of the dominant kernel (the adjoint step)
             roof["traffic"] = t["adjoint_bytes_per_launch"] / 1e9
-            roof["traffic_unit"] = "GB per launch (dram__bytes_read.sum + dram__bytes_write.sum), algorithmic %.2f" % (B_ALG * prm.N / 1e9)
+            roof["traffic_unit"] = "GB per launch (dram__bytes_read.sum + dram__bytes_write.sum), algorithmic %.2f" % (B * prm.N / 1e9)
             roof["traffic_forward"] = t["forward_bytes_per_launch"] / 1e9
 
     # ---- end to end through the host-buffer entry points (pinned host memory, copies inside)

@@ -742,7 +742,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             kE = fE != 0 && fE == fMu;                                     // rho, alpha slot (it + 3) % 3 holds plane it (>= 0)
             kMu = it >= 3 && fMu != 0 && fMu == fM3;
             kLam = it >= 2 && fLam != 0 && fLam == fM3;
-            if (it + 1 < itn) issueU(it + 1);   // needed first ; slot of plane it - 4: its last cross-thread reads were in stage 2 of it - 2
+            if (it + 1 < itn) issueU(it + 1);   // needed first ; slot of plane it - 3: its last cross-thread reads were in stage 2 of it - 1
             if (it + 2 <= itn) issueM(it, fMu, fLam, kMu, kLam);
             if (exa < 0 && it + 2 < itn) issueG(it + 2, fE, 0u, kE);   // exchange CTAs: after stage 2 (its slots are their scratch)
         }

@@ -397,6 +397,15 @@ def gaussian_ball(prm: Params, c, sigma, amp=1.0, cut=3.5) -> np.ndarray:
     return _gaussian_blob(prm, np.asarray(c, dtype=np.float64), sigma, amp, cut)
 
 
+def fluid_version(prob: Problem) -> Problem:
+    """The same workload with the shear modulus set to zero everywhere and the longitudinal speed kept
+    (lambda' = lambda + 2 mu = rho c_l^2): the medium of the paper's H^dagger_{mu=0} ("the shear
+    modulus of the elastic medium was set to zero", the skull's longitudinal speed being a free parameter)."""
+    from dataclasses import replace
+    lam = (prob.lam.astype(np.float64) + 2.0 * prob.mu.astype(np.float64)).astype(np.float32)
+    return replace(prob, name=prob.name + "-fluid", lam=lam, mu=np.zeros_like(prob.mu))
+
+
 def crop(prob: Problem, origin, n, nt: int) -> Problem:
     """Sub-block [z0:z0+n, y0:y0+n, x0:x0+n] of a problem's volumes with the receivers that fall
     inside it (shifted to the block's origin) and `nt` samples — a bounded sample of the same
