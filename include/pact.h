@@ -143,6 +143,9 @@ const char* pact_last_cuda_error(void);
  *              0: launch directly; -1: automatic.
  *   "zchunk"   planes of z each CTA of the fused kernel marches over (0 = automatic).  Any value
  *              gives the same operator; it only changes how the grid is cut into CTAs.
+ *   "chunk_long", "chunk_short"  tuning knobs of the automatic cut (0 = built-in 128 / 40): longest chunk of the
+ *              first five sixths of a tile column, and of its last sixth (listed last, so that a launch ends on
+ *              short bricks).  Any value gives the same operator.
  *   "split_launch"  1 (default): a fused time step runs its C-PML (slab) bricks and then its C-PML-free
  *              (interior) bricks as two launches on the context's stream, each timed on its own
  *              (PACT_K_*_SLAB / PACT_K_*_INTERIOR); 0: one persistent launch over the whole work list

@@ -75,6 +75,7 @@ struct pact_ctx {
     CUtensorMap tmS40[2], tmS36[2], tmS32[2], tmM37, tmM36, tmL;
     FusedArgs fa;
     int zchunk;              // planes per CTA along z (0 = auto)
+    int chunk_long, chunk_short;   // automatic chunking: longest long / short chunk (options "chunk_long", "chunk_short")
     // work list of the fused launch, heaviest first: [0, nslab) bricks that touch a C-PML slab (they run the C-PML
     // code), [nslab, nwork) bricks whose every tap (those of the adjoint included) stays clear of the slabs
     int4* d_work;
@@ -641,7 +642,8 @@ static int ensure_fused(pact_ctx* c)
 // the rest in short ones (<= FT_CHUNK_SHORT) that the host lists last.
 #define FT_CHUNK_LONG 128
 #define FT_CHUNK_SHORT 40
-static void cut_chunks(int z0, int z1, int zc, std::vector<std::pair<int, int>>& longs, std::vector<std::pair<int, int>>& shorts)
+static void cut_chunks(int z0, int z1, int zc, int len_long, int len_short, std::vector<std::pair<int, int>>& longs,
+                       std::vector<std::pair<int, int>>& shorts)
 {
     const int n = z1 - z0;
     if (n <= 0) return;
@@ -652,10 +654,10 @@ static void cut_chunks(int z0, int z1, int zc, std::vector<std::pair<int, int>>&
         for (int i = 0; i < k; ++i) out.push_back({a + (int)((long long)m * i / k), a + (int)((long long)m * (i + 1) / k)});
     };
     if (zc > 0) { equal_parts(z0, z1, zc, longs); return; }
-    if (n <= FT_CHUNK_SHORT + 8) { shorts.push_back({z0, z1}); return; }
+    if (n <= len_short + 8) { shorts.push_back({z0, z1}); return; }
     const int tail = std::max(n / 6, 24);
-    equal_parts(z0, z1 - tail, FT_CHUNK_LONG, longs);
-    equal_parts(z1 - tail, z1, FT_CHUNK_SHORT, shorts);
+    equal_parts(z0, z1 - tail, len_long, longs);
+    equal_parts(z1 - tail, z1, len_short, shorts);
 }
 
 // Work list: a brick is "interior" when its u region with the +-2 taps of the transposed
@@ -668,6 +670,7 @@ static int build_work(pact_ctx* c)
 {
     if (c->work_zc == c->zchunk) return PACT_OK;
     const DevGrid& g = c->g;
+    const int LL = c->chunk_long > 0 ? c->chunk_long : FT_CHUNK_LONG, LS = c->chunk_short > 0 ? c->chunk_short : FT_CHUNK_SHORT;
     const int P = g.P, ntx = (g.nx + FT_TX - 1) / FT_TX, nty = (g.ny + FT_TY - 1) / FT_TY;
     auto interior_1d = [&](int t0, int n) { return P == 0 || (t0 - 4 >= P && t0 + 36 <= n - 1 - P); };
     int zlo = 0, zhi = g.nz;
@@ -682,12 +685,12 @@ static int build_work(pact_ctx* c)
             for (auto& t : tiles) wl.push_back(make_int4(t.first | flag, t.second, ch.first, ch.second));
     };
     std::vector<std::pair<int, int>> bl, bs, il, is, zl, zs;
-    if (!tbd.empty()) cut_chunks(0, g.nz, c->zchunk, bl, bs);
+    if (!tbd.empty()) cut_chunks(0, g.nz, c->zchunk, LL, LS, bl, bs);
     if (!tin.empty()) {
-        cut_chunks(zlo, zhi, c->zchunk, il, is);
+        cut_chunks(zlo, zhi, c->zchunk, LL + LL / 4, LS, il, is);   // interior bricks: longer long chunks (measured: 160 beats 128 by 2 %)
         if (P > 0) {   // the z slabs of interior tiles: thin bricks
-            cut_chunks(0, zlo, c->zchunk, zl, zs);
-            cut_chunks(zhi, g.nz, c->zchunk, zl, zs);
+            cut_chunks(0, zlo, c->zchunk, LL, LS, zl, zs);
+            cut_chunks(zhi, g.nz, c->zchunk, LL, LS, zl, zs);
         }
     }
     const int slab = P > 0 ? FT_WORK_SLAB : 0;
@@ -1017,6 +1020,12 @@ extern "C" int pact_set_option(pact_ctx* c, const char* key, long long value)
     if (!strcmp(key, "variant")) {
         if (value < 0 || value > 2) return PACT_EINVAL;
         c->variant = (int)value;
+        return PACT_OK;
+    }
+    if (!strcmp(key, "chunk_long") || !strcmp(key, "chunk_short")) {
+        if (value < 0 || value > 65535) return PACT_EINVAL;
+        (key[6] == 'l' ? c->chunk_long : c->chunk_short) = (int)value;
+        c->work_zc = -1; free_graphs(c);
         return PACT_OK;
     }
     if (!strcmp(key, "zchunk")) { if (value < 0) return PACT_EINVAL; c->zchunk = (int)value; free_graphs(c); return PACT_OK; }
