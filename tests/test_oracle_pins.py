@@ -546,3 +546,41 @@ def test_adjoint_recursion_matches_eq27():
         o.adj_step()
         o.adj_source(y[m - 1])
     assert np.array_equal(o.adj_image(), want)
+
+
+# ----------------------------------------------------------------------------- projected gradient (oracle/pgd.py)
+
+def test_pgd_oracle_against_dense_matrix():
+    """oracle/pgd.py against plain linear algebra on the dense H of a tiny grid
+    (independent Kronecker assembly, oracle/bruteforce.py): the power iteration converges to the largest eigenvalue
+    of H^T H (numpy SVD), every projected-gradient iterate equals max(0, p - s H^T (H p - d)) computed with the dense
+    matrix, the reported norms are those of the dense residual / update, and with s = 1/||H||^2 the residual never
+    grows (the step is non-expansive)."""
+    from oracle import pgd as opgd
+    pb = synth.random_problem(nx=7, ny=6, nz=5, nt=6, npml=2, L=4, seed=17)
+    H = bf.system_matrix(pb)                                  # (nt L) x N
+    o = Oracle.from_problem(pb)
+    rng = np.random.default_rng(17)
+    shape = pb.p0.shape
+    s2_true = np.linalg.svd(H, compute_uv=False)[0] ** 2
+    s2, v = opgd.power_iteration(o, rng.standard_normal(shape), iters=200)
+    assert abs(s2 - s2_true) <= 1e-6 * s2_true                # converged (gap-dependent, hence 200 iterations)
+    assert abs(np.linalg.norm(v) - 1.0) <= 1e-12
+    s2_8, _ = opgd.power_iteration(o, rng.standard_normal(shape), iters=8)
+    assert 0.5 * s2_true <= s2_8 <= s2_true * (1 + 1e-12)     # a Rayleigh-type estimate never exceeds the true value
+    p_true = np.maximum(rng.standard_normal(shape), 0.0)
+    d = (H @ p_true.ravel()).reshape(pb.prm.nt, pb.L) + 0.01 * rng.standard_normal((pb.prm.nt, pb.L))
+    step = 1.0 / s2_true
+    its, res, upd = opgd.pgd(o, np.zeros(shape), d, step, 5)
+    p = np.zeros(H.shape[1])
+    for k in range(5):
+        r = H @ p - d.ravel()
+        q = np.maximum(p - step * (H.T @ r), 0.0)
+        assert abs(res[k] - np.linalg.norm(r)) <= 1e-12 * np.linalg.norm(r)
+        assert abs(upd[k] - np.linalg.norm(q - p)) <= 1e-10 * max(np.linalg.norm(q - p), 1e-30)
+        assert np.abs(its[k].ravel() - q).max() <= 1e-12 * max(np.abs(q).max(), 1e-30)
+        p = q
+    assert all(res[k + 1] <= res[k] * (1 + 1e-12) for k in range(4))
+    # without the projection the same code is plain gradient descent (Landweber)
+    its_u, _, _ = opgd.pgd(o, np.zeros(shape), d, step, 1, nonneg=False)
+    assert np.abs(its_u[0].ravel() - (-step) * (H.T @ (-d.ravel()))).max() <= 1e-12 * np.abs(its_u[0]).max()
