@@ -422,9 +422,10 @@ def main():
         roof["traffic_source"] = src
         if t:
             # per launch of the dominant kernel (the adjoint step)
-            roof["traffic"] = t["adjoint_bytes_per_launch"] / 1e9
+            pre = "acoustic_" if args.acoustic else ""
+            roof["traffic"] = t[pre + "adjoint_bytes_per_launch"] / 1e9
             roof["traffic_unit"] = "GB per launch (dram__bytes_read.sum + dram__bytes_write.sum), algorithmic %.2f" % (B * prm.N / 1e9)
-            roof["traffic_forward"] = t["forward_bytes_per_launch"] / 1e9
+            roof["traffic_forward"] = t[pre + "forward_bytes_per_launch"] / 1e9
 
     # ---- end to end through the host-buffer entry points (pinned host memory, copies inside)
     e2e = None
