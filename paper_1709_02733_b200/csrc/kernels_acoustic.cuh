@@ -1,8 +1,8 @@
 // kernels_acoustic.cuh — the fluid-only specialisation of the fused step: H and H^T of a medium with
 // mu = 0 everywhere (the paper's H^dagger_{mu=0}: the skull treated as a fluid).
 //
-// With mu = 0 the three normal stresses stay equal and the shear stresses stay zero (Eq. 46 with M_jk = 0; pinned for the
-// oracle by tests/test_oracle_pins.py::test_fluid_special_case_matches_textbook_acoustics), so the state collapses to
+// With mu = 0 the three normal stresses stay equal and the shear stresses stay zero (Eq. 46 with M_jk = 0; DESIGN.md section 3,
+// row "mu = 0"), so the state collapses to
 // one stress field s (= sigma11 = sigma22 = sigma33, kept in the S11 slot of the state) and the three velocities:
 //     u_a <- J_a u_a + B_a (D+_a s + phi_aa)            a = x, y, z          (Eq. 46a,b)
 //     s   <- s + Ll (sum_a D-_a u_a + psi_aa)                                (Eq. 46c,d ; lambda only)
