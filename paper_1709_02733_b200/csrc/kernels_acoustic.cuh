@@ -140,7 +140,7 @@ __device__ __forceinline__ void acoustic_brick(float* __restrict__ sm, const CUt
         tma_plane(&tmS36, sm + AC_OFF_UR + (2 * AC_RING + c % AC_RING) * FT_UPL, bar, cx40, cy36, cz0 + c, U3);
     };
 
-    if (tid == 0) {
+    if (tid == FT_PROD) {
         const unsigned f0 = mflag_at(0), f1 = mflag_at(1), f2 = mflag_at(2);
         fh = (unsigned long long)f2 | ((unsigned long long)f1 << 8) | ((unsigned long long)f0 << 16) | ((unsigned long long)mflag_at(-1) << 24);
         issueG(0, f1, f0, false); issueG(1, f2, 0u, false);
@@ -169,7 +169,7 @@ __device__ __forceinline__ void acoustic_brick(float* __restrict__ sm, const CUt
     for (int it = 0; it < itn; ++it) {
         const int kk = zb - 2 + it;
         unsigned fnew = 0;
-        if (tid == 0) fnew = mflag_at(it + 3);
+        if (tid == FT_PROD) fnew = mflag_at(it + 3);
         // forward C-PML: phi11 (x), phi22 (y), phi33 (z) of the own quad at plane kk, issued ahead of the wait
         float4 pm0 = z4, pm1 = z4, pm2 = z4;
         if (MODE == FM_FWD) {
@@ -306,7 +306,7 @@ __device__ __forceinline__ void acoustic_brick(float* __restrict__ sm, const CUt
         __syncthreads();
         unsigned fE = 0, fLam = 0;
         bool kE = false, kLam = false;
-        if (tid == 0) {
+        if (tid == FT_PROD) {
             fh = (fh << 8) | fnew;
             fE = (unsigned)fh & 0xffu; fLam = (unsigned)(fh >> 32) & 0xffu;
             const unsigned fIt = (unsigned)(fh >> 24) & 0xffu, fM3 = (unsigned)(fh >> 48) & 0xffu;

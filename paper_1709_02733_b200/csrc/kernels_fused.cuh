@@ -45,6 +45,11 @@
 #define FT_RH 37                      // rows of the rho / alpha planes: u region + 1
 #define FT_RPL 1504                   // floats per rho / alpha plane buffer (40*37 = 1480, padded to 128 B)
 #define FT_LPL (FT_TX * FT_TY)        // floats per lambda plane (the tile itself)
+// The thread that issues every TMA of the loop.  Warp 11 holds only 8 quads of the u region's last ring row (no stage 2
+// work), so its spare lane 12 runs the ~250 instructions of the issue block off the critical path of the other warps.
+#ifndef FT_PROD
+#define FT_PROD 364
+#endif
 #define FT_RING 4                     // u planes in the ring: ks .. ks+2 and the slot u_old(kk+1) is landing in
 
 // shared memory map (floats).  Planes are only as tall as their readers need: s11, s13 (x neighbours only) and
@@ -75,6 +80,7 @@
 #define FM_ADJ 2       // W'^T : Eq. 61, memory variables (tilde form) applied before differencing
 
 #define FT_WORK_SLAB 0x10000           // flag in work[b].x: the brick touches a C-PML slab (runs the launch's C-PML code)
+#define FT_WORK_NOEDGE 0x20000         // flag in work[b].x: u region, taps and planes zb-2 .. ze+1 lie inside the grid (no lane masks)
 
 struct FusedArgs {
     int nx, ny, nz;
@@ -135,6 +141,13 @@ __device__ __forceinline__ void tma_plane(const CUtensorMap* tm, float* dst, uin
         "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
         ::"r"(smem_u32(dst)), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar))
         : "memory");
+}
+
+// the same box requested into L2 only (no shared-memory destination, no barrier)
+__device__ __forceinline__ void tma_prefetch_plane(const CUtensorMap* tm, int c0, int c1, int c2, int c3)
+{
+    asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];"
+                 ::"l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
 }
 
 // ---- float4 helpers -----------------------------------------------------------------------------
@@ -218,10 +231,11 @@ __device__ __forceinline__ void ldg4_into(float4& v, const float* p, bool pred)
 }
 __device__ __forceinline__ void stg4(float* p, float4 v) { *reinterpret_cast<float4*>(p) = v; }
 
-// store the in-grid lanes of a quad starting at column x
+// store the in-grid lanes of a quad starting at column x (EDGE = false: the whole quad is in the grid)
+template <bool EDGE = true>
 __device__ __forceinline__ void store_quad(float* p, float4 v, int x, int nx)
 {
-    if (x + 3 < nx) { stg4(p, v); return; }
+    if (!EDGE || x + 3 < nx) { stg4(p, v); return; }
     if (x < nx) p[0] = v.x;
     if (x + 1 < nx) p[1] = v.y;
     if (x + 2 < nx) p[2] = v.z;
@@ -353,7 +367,9 @@ __device__ __forceinline__ float4 adj_own_x(float4 Told, float* To, long long i,
 // The fused step.  MODE selects the C-PML code carried by the launch (FM_*); see DESIGN.md for the
 // index algebra.  Relative plane j <-> z = zb - 2 + j ; iteration `it` computes u(kk = zb - 2 + it)
 // and sigma(ks = kk - 2).
-template <int MODE>
+// EDGE = false: the host vouches (FT_WORK_NOEDGE) that nothing this brick touches sticks out of the grid, so the lane
+// masks, the in-grid tests of the stores and the z range tests are compiled out.
+template <int MODE, bool EDGE>
 __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtensorMap& tmS40, const CUtensorMap& tmS36,
                                             const CUtensorMap& tmM37, const CUtensorMap& tmM36, const CUtensorMap& tmL,
                                             const CUtensorMap& tmS32, const FusedArgs& a, const int4 wk, const bool first)
@@ -372,19 +388,19 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
     const bool act1 = tid < 360;
     const int qx = tid % 10, r = tid / 10;
     const int x = x0 - 4 + 4 * qx, y = y0 - 2 + r;
-    const bool inner = act1 && qx >= 1 && qx <= 8 && r >= 2 && r < 34 && x < a.nx && y < a.ny;
+    const bool inner = act1 && qx >= 1 && qx <= 8 && r >= 2 && r < 34 && (!EDGE || (x < a.nx && y < a.ny));
     const int q = tid + 20;                 // quad index in a 40x40 plane (two rows further down)
     const int uq = tid;                     // quad index in a 40x36 plane
     const int mq = (r - 2) * 9 + (qx - 1);  // quad index in a mu plane (inner threads)
     // own-column global loads are legal where the padded box has storage
-    const bool ld_ok = act1 && (y + PACT_HALO_Y < a.ny + 2 * PACT_HALO_Y) && (x + 3 + PACT_HALO_X < (int)a.sy);
+    const bool ld_ok = act1 && (!EDGE || ((y + PACT_HALO_Y < a.ny + 2 * PACT_HALO_Y) && (x + 3 + PACT_HALO_X < (int)a.sy)));
     const long long gxy = (long long)y * a.sy + x;
     // lanes of the quad that are grid points (u outside the grid is zero: reading G9)
     const bool yin = (unsigned)y < (unsigned)a.ny;
     const bool m0 = yin && (unsigned)x < (unsigned)a.nx, m1 = yin && (unsigned)(x + 1) < (unsigned)a.nx;
     const bool m2 = yin && (unsigned)(x + 2) < (unsigned)a.nx, m3 = yin && (unsigned)(x + 3) < (unsigned)a.nx;
     // the CTA's u region sticks out of the grid in x or y (then lanes are masked every plane)
-    const bool edge_xy = x0 == 0 || y0 == 0 || x0 + FT_TX + 4 > a.nx || y0 + FT_TY + 2 > a.ny;
+    const bool edge_xy = EDGE && (x0 == 0 || y0 == 0 || x0 + FT_TX + 4 > a.nx || y0 + FT_TY + 2 > a.ny);
 
     // C-PML: does the CTA's region (plus the taps of the adjoint) touch the x / y slabs; own-quad slab positions
     const bool pml = MODE != FM_PLAIN && a.P > 0;
@@ -483,7 +499,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
         tma_plane(&tmS36, sm + FT_OFF_UR + (2 * FT_RING + c % FT_RING) * FT_UPL, bar, cx40, cy36, cz0 + c, U3);
     };
 
-    if (tid == 0) {
+    if (tid == FT_PROD) {
         const unsigned f0 = mflag_at(0), f1 = mflag_at(1), f2 = mflag_at(2);
         fh = (unsigned long long)f2 | ((unsigned long long)f1 << 8) | ((unsigned long long)f0 << 16) | ((unsigned long long)mflag_at(-1) << 24);
         issueG(0, f1, f0, false); issueG(1, f2, 0u, false); issueU(0);
@@ -525,7 +541,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
     for (int it = 0; it < itn; ++it) {
         const int kk = zb - 2 + it;
         unsigned fnew = 0;      // thread 0: material flag of plane it + 3, fetched half an iteration before its use
-        if (tid == 0) fnew = mflag_at(it + 3);
+        if (tid == FT_PROD) fnew = mflag_at(it + 3);
         // forward C-PML: the nine phi of this thread's quad at plane kk, issued together ahead of the wait
         // (one exposed latency per stage instead of nine serialised ones)
         float4 pm[9];
@@ -560,7 +576,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
 
         const int s3 = it % 3, s3n = (it + 1) % 3;
         float4 f13 = z4, f23 = z4, f33 = z4;     // fresh window entries: s13, s23 at kk+1, s33 at kk+2
-        const bool zin = (unsigned)kk < (unsigned)a.nz;
+        const bool zin = !EDGE || (unsigned)kk < (unsigned)a.nz;
         // ------------------------------------------------------------------ stage 1: u(kk)
         // Adjoint slab CTAs: X = a T of the own quad for the three terms of the exchange axis, T <- b T + s, into the ring
         // slot that u_old(kk+1) will land in after the barrier (free: the closing barrier of the previous iteration's
@@ -680,7 +696,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                 const float4 rzp = ld4s(Rbase + s3n * FT_RPL, uq), azp = ld4s(Abase + s3n * FT_RPL, uq);
                 n3 = fma4(fma4(mh, a0 + azp, one), *reinterpret_cast<const float4*>(R3), (kB * rcp4(r0 + rzp)) * (t1 + t2 + t3));
             }
-            if (edge_xy || !zin) {
+            if (EDGE && (edge_xy || !zin)) {
                 if (!(zin && m0)) { n1.x = 0.0f; n2.x = 0.0f; n3.x = 0.0f; }
                 if (!(zin && m1)) { n1.y = 0.0f; n2.y = 0.0f; n3.y = 0.0f; }
                 if (!(zin && m2)) { n1.z = 0.0f; n2.z = 0.0f; n3.z = 0.0f; }
@@ -693,9 +709,9 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             const long long g = (long long)kk * a.sz + gxy;
             if (wr1) {
-                store_quad(a.out + U1 * box + g, n1, x, a.nx);
-                store_quad(a.out + U2 * box + g, n2, x, a.nx);
-                store_quad(a.out + U3 * box + g, n3, x, a.nx);
+                store_quad<EDGE>(a.out + U1 * box + g, n1, x, a.nx);
+                store_quad<EDGE>(a.out + U2 * box + g, n2, x, a.nx);
+                store_quad<EDGE>(a.out + U3 * box + g, n3, x, a.nx);
             }
         }
         // forward C-PML: the nine psi of the quad at plane ks = kk - 2, issued ahead of the barrier
@@ -735,7 +751,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
         // thread 0: flags of planes it + 3 (E), it (mu), it - 1 (lambda) and of the planes that filled their slots last
         unsigned fE = 0, fMu = 0, fLam = 0;
         bool kE = false, kMu = false, kLam = false;
-        if (tid == 0) {
+        if (tid == FT_PROD) {
             fh = (fh << 8) | fnew;
             fE = (unsigned)fh & 0xffu; fMu = (unsigned)(fh >> 24) & 0xffu; fLam = (unsigned)(fh >> 32) & 0xffu;
             const unsigned fM3 = (unsigned)(fh >> 48) & 0xffu;             // plane it - 3: previous tenant of the mu and lambda slots
@@ -743,6 +759,13 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             kMu = it >= 3 && fMu != 0 && fMu == fM3;
             kLam = it >= 2 && fLam != 0 && fLam == fM3;
             if (it + 1 < itn) issueU(it + 1);   // needed first ; slot of plane it - 3: its last cross-thread reads were in stage 2 of it - 1
+#ifdef FT_EXP_PFU
+            if (it + FT_EXP_PFU < itn) {
+                tma_prefetch_plane(&tmS36, cx40, cy36, cz0 + it + FT_EXP_PFU, U1);
+                tma_prefetch_plane(&tmS36, cx40, cy36, cz0 + it + FT_EXP_PFU, U2);
+                tma_prefetch_plane(&tmS36, cx40, cy36, cz0 + it + FT_EXP_PFU, U3);
+            }
+#endif
             if (it + 2 <= itn) issueM(it, fMu, fLam, kMu, kLam);
             if (exa < 0 && it + 2 < itn) issueG(it + 2, fE, 0u, kE);   // exchange CTAs: after stage 2 (its slots are their scratch)
         }
@@ -880,16 +903,16 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             const float4 n13 = fma4(mxz, g13 + g31, w13a);
             const float4 n23 = fma4(myz, g23 + g32, w23a);
             const long long g = (long long)ks * a.sz + gxy;
-            store_quad(a.out + S11 * box + g, n11, x, a.nx);
-            store_quad(a.out + S22 * box + g, n22, x, a.nx);
-            store_quad(a.out + S33 * box + g, n33, x, a.nx);
-            store_quad(a.out + S12 * box + g, n12, x, a.nx);
-            store_quad(a.out + S13 * box + g, n13, x, a.nx);
-            store_quad(a.out + S23 * box + g, n23, x, a.nx);
+            store_quad<EDGE>(a.out + S11 * box + g, n11, x, a.nx);
+            store_quad<EDGE>(a.out + S22 * box + g, n22, x, a.nx);
+            store_quad<EDGE>(a.out + S33 * box + g, n33, x, a.nx);
+            store_quad<EDGE>(a.out + S12 * box + g, n12, x, a.nx);
+            store_quad<EDGE>(a.out + S13 * box + g, n13, x, a.nx);
+            store_quad<EDGE>(a.out + S23 * box + g, n23, x, a.nx);
         }
         if (exa >= 0) {   // every thread is done with the exchange planes: now the group that refills them may go
             __syncthreads();
-            if (tid == 0 && it + 2 < itn) issueG(it + 2, fE, 0u, kE);
+            if (tid == FT_PROD && it + 2 < itn) issueG(it + 2, fE, 0u, kE);
         }
         u3m2 = u3m1; u1m1 = cc1; u2m1 = cc2; u3m1 = cc3;
         // slide the z windows
@@ -921,8 +944,9 @@ k_step(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUtens
         const int b = *s_next;
         if (b >= n) break;
         const int4 wk = __ldg(a.work + a.work_begin + b);
-        if (MODE != FM_PLAIN && (wk.x & FT_WORK_SLAB)) fused_brick<MODE>(sm, tmS40, tmS36, tmM37, tmM36, tmL, tmS32, a, wk, first);
-        else fused_brick<FM_PLAIN>(sm, tmS40, tmS36, tmM37, tmM36, tmL, tmS32, a, wk, first);
+        if (MODE != FM_PLAIN && (wk.x & FT_WORK_SLAB)) fused_brick<MODE, true>(sm, tmS40, tmS36, tmM37, tmM36, tmL, tmS32, a, wk, first);
+        else if (wk.x & FT_WORK_NOEDGE) fused_brick<FM_PLAIN, false>(sm, tmS40, tmS36, tmM37, tmM36, tmL, tmS32, a, wk, first);
+        else fused_brick<FM_PLAIN, true>(sm, tmS40, tmS36, tmM37, tmM36, tmL, tmS32, a, wk, first);
         first = false;
         // generic-proxy writes of this brick (tables, exchange planes) precede the TMA writes of the next one
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");

@@ -682,7 +682,12 @@ static int build_work(pact_ctx* c)
     std::vector<int4> wl;
     auto add = [&](const std::vector<std::pair<int, int>>& tiles, const std::vector<std::pair<int, int>>& chunks, int flag) {
         for (auto& ch : chunks)
-            for (auto& t : tiles) wl.push_back(make_int4(t.first | flag, t.second, ch.first, ch.second));
+            for (auto& t : tiles) {
+                // nothing the brick touches sticks out of the grid: its instance without lane masks (FT_WORK_NOEDGE)
+                const int x0 = t.first * FT_TX, y0 = t.second * FT_TY;
+                const bool clear = x0 >= 4 && x0 + FT_TX + 4 <= g.nx && y0 >= 4 && y0 + FT_TY + 4 <= g.ny && ch.first >= 4 && ch.second + 4 <= g.nz;
+                wl.push_back(make_int4(t.first | flag | (clear && !flag ? FT_WORK_NOEDGE : 0), t.second, ch.first, ch.second));
+            }
     };
     std::vector<std::pair<int, int>> bl, bs, il, is, zl, zs;
     if (!tbd.empty()) cut_chunks(0, g.nz, c->zchunk, LL, LS, bl, bs);
