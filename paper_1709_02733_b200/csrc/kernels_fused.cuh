@@ -50,7 +50,13 @@
 #ifndef FT_PROD
 #define FT_PROD 364
 #endif
-#define FT_RING 4                     // u planes in the ring: ks .. ks+2 and the slot u_old(kk+1) is landing in
+// Where stage 2 finds the old s11, s22, s12 of its plane (own quad): 0 = s11, s22 as 32 x 32 tile planes by TMA and s12 by
+// an own-column load (u ring of 4) ; 1 = three own-column loads ; 2 = parked in tensor memory by stage 1 of the same
+// thread two iterations earlier.  1 and 2 free the tile planes for a fifth ring slot: u_old is then requested a whole
+// iteration earlier.
+// The mode is a property of the kernel (template parameter SOM of the brick routine, FusedMap below).
+#define FT_RING 4                     // mode 0: u planes in the ring: ks .. ks+2 and the slot u_old(kk+1) is landing in
+#define FT_TMEM_COLS 128              // tensor-memory columns allocated per CTA (mode 2): 3 warps per lane quarter x 36
 
 // shared memory map (floats).  Planes are only as tall as their readers need: s11, s13 (x neighbours only) and
 // s33 (own column) cover the u region (36 rows), rho / alpha one row more, s22, s12, s23 the full 40.
@@ -72,7 +78,29 @@
 #define FT_OFF_XT (FT_OFF_END + 16)   // after 8 mbarriers (64 B)
 #define FT_OFF_YT (FT_OFF_XT + 4 * FT_TABW)
 #define FT_OFF_ZT (FT_OFF_YT + 4 * FT_TABW)
-#define FT_SMEM_BYTES ((FT_OFF_ZT + 4 * FT_ZRING + 4) * 4)   // + the work-queue ticket
+// the tail of the map for a given SO mode: modes 1, 2 trade the four old-stress tile planes for a fifth ring slot
+template <int SOM>
+struct FusedMap {
+    static constexpr int RING = SOM == 0 ? 4 : 5;      // ... and the slots of u_old(kk+1) (landed), u_old(kk+2) (landing)
+    static constexpr int ULEAD = RING - 3;             // u_old(c) is requested after the block barrier of iteration c - ULEAD
+    static constexpr int OFF_UR = FT_OFF_SO + (SOM == 0 ? 4 : 0) * FT_LPL;
+    static constexpr int OFF_END = OFF_UR + 3 * RING * FT_UPL;
+    static constexpr int OFF_XT = OFF_END + 16;
+    static constexpr int OFF_YT = OFF_XT + 4 * FT_TABW;
+    static constexpr int OFF_ZT = OFF_YT + 4 * FT_TABW;
+    static constexpr int OFF_TICKET = OFF_ZT + 4 * FT_ZRING;   // the work-queue ticket, then the tensor-memory base address
+    static constexpr int BYTES = (OFF_TICKET + 4) * 4;
+};
+#define FT_SMEM_BYTES (FusedMap<2>::BYTES > FusedMap<0>::BYTES ? FusedMap<2>::BYTES : FusedMap<0>::BYTES)
+static_assert(FT_SMEM_BYTES <= 232448, "shared-memory map exceeds 227 KB");
+// SO mode of the kernel that carries C-PML mode MODE: the C-PML kernels are at the register limit already
+#ifndef FT_SOM_PML
+#define FT_SOM_PML 0
+#endif
+#ifndef FT_SOM_PLAIN
+#define FT_SOM_PLAIN 2
+#endif
+#define FT_SOM(MODE) ((MODE) == FM_PLAIN ? FT_SOM_PLAIN : FT_SOM_PML)
 
 // kernel modes: which C-PML code a launch carries (CTAs away from the slabs skip it at run time)
 #define FM_PLAIN 0     // no C-PML (npml = 0)
@@ -143,12 +171,20 @@ __device__ __forceinline__ void tma_plane(const CUtensorMap* tm, float* dst, uin
         : "memory");
 }
 
-// the same box requested into L2 only (no shared-memory destination, no barrier)
-__device__ __forceinline__ void tma_prefetch_plane(const CUtensorMap* tm, int c0, int c1, int c2, int c3)
+// ---- tensor memory as per-thread scratch (SASS: STTM / LDTM): 32x32b = lane <-> thread, 4 consecutive 32-bit columns
+__device__ __forceinline__ void tmem_st4(uint32_t taddr, float4 v)
 {
-    asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];"
-                 ::"l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};"
+                 ::"r"(taddr), "r"(__float_as_uint(v.x)), "r"(__float_as_uint(v.y)), "r"(__float_as_uint(v.z)), "r"(__float_as_uint(v.w)) : "memory");
 }
+__device__ __forceinline__ float4 tmem_ld4(uint32_t taddr)
+{
+    uint32_t x, y, z, w;
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(x), "=r"(y), "=r"(z), "=r"(w) : "r"(taddr) : "memory");
+    return make_float4(__uint_as_float(x), __uint_as_float(y), __uint_as_float(z), __uint_as_float(w));
+}
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
 // ---- float4 helpers -----------------------------------------------------------------------------
 __device__ __forceinline__ float4 ld4s(const float* p, int quad) { return *reinterpret_cast<const float4*>(p + 4 * quad); }
@@ -369,15 +405,18 @@ __device__ __forceinline__ float4 adj_own_x(float4 Told, float* To, long long i,
 // and sigma(ks = kk - 2).
 // EDGE = false: the host vouches (FT_WORK_NOEDGE) that nothing this brick touches sticks out of the grid, so the lane
 // masks, the in-grid tests of the stores and the z range tests are compiled out.
-template <int MODE, bool EDGE>
+template <int MODE, bool EDGE, int SOM>
 __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtensorMap& tmS40, const CUtensorMap& tmS36,
                                             const CUtensorMap& tmM37, const CUtensorMap& tmM36, const CUtensorMap& tmL,
-                                            const CUtensorMap& tmS32, const FusedArgs& a, const int4 wk, const bool first)
+                                            const CUtensorMap& tmS32, const FusedArgs& a, const int4 wk, const bool first,
+                                            const uint32_t tmem_base)
 {
-    uint64_t* bars = reinterpret_cast<uint64_t*>(sm + FT_OFF_END);
+    constexpr int RING = FusedMap<SOM>::RING, ULEAD = FusedMap<SOM>::ULEAD, OFF_UR = FusedMap<SOM>::OFF_UR;
+    constexpr int OFF_END = FusedMap<SOM>::OFF_END, OFF_XT = FusedMap<SOM>::OFF_XT, OFF_YT = FusedMap<SOM>::OFF_YT, OFF_ZT = FusedMap<SOM>::OFF_ZT;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(sm + OFF_END);
     uint64_t* barG = bars;        // [2]  everything first read by stage 1 of iteration c -> slot c & 1
     uint64_t* barM = bars + 2;    // [3]  mu of plane j -> slot j % 3
-    uint64_t* barU = bars + 5;    // [2]  u_old of plane c, landed in ring slot c % FT_RING -> barrier c & 1
+    uint64_t* barU = bars + 5;    // [2]  u_old of plane c, landed in ring slot c % RING -> barrier c & 1
 
     const int tid = threadIdx.x;
     const int zb = wk.z, ze = wk.w;
@@ -391,6 +430,10 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
     const bool inner = act1 && qx >= 1 && qx <= 8 && r >= 2 && r < 34 && (!EDGE || (x < a.nx && y < a.ny));
     const int q = tid + 20;                 // quad index in a 40x40 plane (two rows further down)
     const int uq = tid;                     // quad index in a 40x36 plane
+    // SOM 2: the thread's tensor-memory scratch (lane = its lane in the warp's lane quarter ; 36 columns per warp:
+    // [plane % 3][s11, s22, s12][4]).  Warp 11 holds no tile quad and takes no part (its u-region lanes diverge).
+    const bool tmw = SOM == 2 && tid < 352;
+    const uint32_t tm0 = tmem_base + ((uint32_t)((tid >> 5) & 3) << 21) + (uint32_t)(tid >> 7) * 36u;
     const int mq = (r - 2) * 9 + (qx - 1);  // quad index in a mu plane (inner threads)
     // own-column global loads are legal where the padded box has storage
     const bool ld_ok = act1 && (!EDGE || ((y + PACT_HALO_Y < a.ny + 2 * PACT_HALO_Y) && (x + 3 + PACT_HALO_X < (int)a.sy)));
@@ -423,12 +466,12 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
     if (pml) {   // stage the C-PML tables: x / y windows and the first planes of the z ring (zeros outside the grid)
         for (int i = tid; i < 4 * FT_TABW; i += FT_NT) {
             const int t = i / FT_TABW, o = i % FT_TABW - 8;
-            sm[FT_OFF_XT + i] = (unsigned)(x0 + o) < (unsigned)a.nx ? __ldg(a.tab[0][t] + x0 + o) : 0.0f;
-            sm[FT_OFF_YT + i] = (unsigned)(y0 + o) < (unsigned)a.ny ? __ldg(a.tab[1][t] + y0 + o) : 0.0f;
+            sm[OFF_XT + i] = (unsigned)(x0 + o) < (unsigned)a.nx ? __ldg(a.tab[0][t] + x0 + o) : 0.0f;
+            sm[OFF_YT + i] = (unsigned)(y0 + o) < (unsigned)a.ny ? __ldg(a.tab[1][t] + y0 + o) : 0.0f;
         }
         if (tid < 4 * 12) {     // planes zb - 10 .. zb + 1 ; the loop adds plane kk + 3 = zb + 1 + it every iteration
             const int t = tid / 12, z = zb - 10 + tid % 12;
-            sm[FT_OFF_ZT + t * FT_ZRING + (z & (FT_ZRING - 1))] = (unsigned)z < (unsigned)a.nz ? __ldg(a.tab[2][t] + z) : 0.0f;
+            sm[OFF_ZT + t * FT_ZRING + (z & (FT_ZRING - 1))] = (unsigned)z < (unsigned)a.nz ? __ldg(a.tab[2][t] + z) : 0.0f;
         }
     }
     if (tid == 0) {   // fresh barriers per brick (every transaction of the previous brick was waited for)
@@ -481,28 +524,31 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
     // flags of planes j (mu) and j - 1 (lambda) ; keep*: the slot holds the same palette plane already
     auto issueM = [&](int j, unsigned fmu, unsigned flam, bool keep_mu, bool keep_lam) {
         uint64_t* bar = &barM[j % 3];
-        mbar_expect_tx(bar, ((keep_mu ? 0 : FT_MW * FT_MH) + (keep_lam ? 2 : 3) * FT_LPL) * 4);
+        mbar_expect_tx(bar, ((keep_mu ? 0 : FT_MW * FT_MH) + ((keep_lam ? 0 : 1) + (SOM == 0 ? 2 : 0)) * FT_LPL) * 4);
         if (!keep_mu) tma_plane(&tmM36, sm + FT_OFF_MU + (j % 3) * FT_MPL, bar, cxm, cym, mz(j, fmu), 1);
         // lambda of plane j - 1 (read by stage 2 of iteration j + 1, which waits on this barrier) -> slot (j - 1) & 1
         if (!keep_lam) tma_plane(&tmL, sm + FT_OFF_LAM + ((j + 1) & 1) * FT_LPL, bar, cxm, cym, mz(j - 1, flam), 0);
         // and the old s11, s22 of that plane (the tile itself): they are the sigma(ks) that stage 2 adds to
-        tma_plane(&tmS32, sm + FT_OFF_SO + (2 * ((j + 1) & 1) + 0) * FT_LPL, bar, cxm, cym, cz0 + j - 1, S11);
-        tma_plane(&tmS32, sm + FT_OFF_SO + (2 * ((j + 1) & 1) + 1) * FT_LPL, bar, cxm, cym, cz0 + j - 1, S22);
+        if (SOM == 0) {
+            tma_plane(&tmS32, sm + FT_OFF_SO + (2 * ((j + 1) & 1) + 0) * FT_LPL, bar, cxm, cym, cz0 + j - 1, S11);
+            tma_plane(&tmS32, sm + FT_OFF_SO + (2 * ((j + 1) & 1) + 1) * FT_LPL, bar, cxm, cym, cz0 + j - 1, S22);
+        }
     };
 
     // u_old(c) lands in the ring slot that u_new(c) will overwrite in place (own quads only)
     auto issueU = [&](int c) {
         uint64_t* bar = &barU[c & 1];
         mbar_expect_tx(bar, 3 * FT_UPL * 4);
-        tma_plane(&tmS36, sm + FT_OFF_UR + (0 * FT_RING + c % FT_RING) * FT_UPL, bar, cx40, cy36, cz0 + c, U1);
-        tma_plane(&tmS36, sm + FT_OFF_UR + (1 * FT_RING + c % FT_RING) * FT_UPL, bar, cx40, cy36, cz0 + c, U2);
-        tma_plane(&tmS36, sm + FT_OFF_UR + (2 * FT_RING + c % FT_RING) * FT_UPL, bar, cx40, cy36, cz0 + c, U3);
+        tma_plane(&tmS36, sm + OFF_UR + (0 * RING + c % RING) * FT_UPL, bar, cx40, cy36, cz0 + c, U1);
+        tma_plane(&tmS36, sm + OFF_UR + (1 * RING + c % RING) * FT_UPL, bar, cx40, cy36, cz0 + c, U2);
+        tma_plane(&tmS36, sm + OFF_UR + (2 * RING + c % RING) * FT_UPL, bar, cx40, cy36, cz0 + c, U3);
     };
 
     if (tid == FT_PROD) {
         const unsigned f0 = mflag_at(0), f1 = mflag_at(1), f2 = mflag_at(2);
         fh = (unsigned long long)f2 | ((unsigned long long)f1 << 8) | ((unsigned long long)f0 << 16) | ((unsigned long long)mflag_at(-1) << 24);
         issueG(0, f1, f0, false); issueG(1, f2, 0u, false); issueU(0);
+        if (ULEAD > 1) issueU(1);
     }
 
     // register windows along z (own column)
@@ -531,9 +577,9 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
     const float* Rbase = sm + FT_OFF_RHO;
     const float* Abase = sm + FT_OFF_ALP;
     // C-PML tables in shared memory, pre-offset: XT(t)[x], YT(t)[y], ZT(t)[z & 15] (t = T_A_INT ..)
-    const float* xt0 = sm + FT_OFF_XT + 8 - x0;
-    const float* yt0 = sm + FT_OFF_YT + 8 - y0;
-    const float* zt0 = sm + FT_OFF_ZT;
+    const float* xt0 = sm + OFF_XT + 8 - x0;
+    const float* yt0 = sm + OFF_YT + 8 - y0;
+    const float* zt0 = sm + OFF_ZT;
 #define XT(t) (xt0 + (t) * FT_TABW)
 #define YT(t) (yt0 + (t) * FT_TABW)
 #define ZT(t) (zt0 + (t) * FT_ZRING)
@@ -581,7 +627,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
         // Adjoint slab CTAs: X = a T of the own quad for the three terms of the exchange axis, T <- b T + s, into the ring
         // slot that u_old(kk+1) will land in after the barrier (free: the closing barrier of the previous iteration's
         // stage 2 was passed by every thread).
-        float* const SC1 = sm + FT_OFF_UR + ((it + 1) % FT_RING) * FT_UPL;     // + f * FT_RING * FT_UPL
+        float* const SC1 = sm + OFF_UR + ((it + ULEAD) % RING) * FT_UPL;     // + f * RING * FT_UPL
         if (exa >= 0) {
             if (act1) {
                 float4 X0 = z4, X1 = z4, X2 = z4;
@@ -602,9 +648,9 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                         X2 = adj_own_x(e1[2], a.mvo[16], ie1, se1, ah, bh, w23c, wr);
                     }
                 }
-                *reinterpret_cast<float4*>(SC1 + 0 * FT_RING * FT_UPL + 4 * uq) = X0;
-                *reinterpret_cast<float4*>(SC1 + 1 * FT_RING * FT_UPL + 4 * uq) = X1;
-                *reinterpret_cast<float4*>(SC1 + 2 * FT_RING * FT_UPL + 4 * uq) = X2;
+                *reinterpret_cast<float4*>(SC1 + 0 * RING * FT_UPL + 4 * uq) = X0;
+                *reinterpret_cast<float4*>(SC1 + 1 * RING * FT_UPL + 4 * uq) = X1;
+                *reinterpret_cast<float4*>(SC1 + 2 * RING * FT_UPL + 4 * uq) = X2;
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // TMA overwrites these planes later
             }
             __syncthreads();
@@ -632,13 +678,16 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             const float4 r0 = ld4s(PR, uq), a0 = ld4s(PA, uq);
             const float4 one = f4(1.0f), mh = f4(-0.5f);
             const float4 c12 = ld4s(P12, q);
+            const uint32_t tms = tm0 + (uint32_t)(it % 3) * 12u;      // SOM 2: this plane's parking columns
+            if (tmw) tmem_st4(tms + 8u, c12);
             float4 n1, n2, n3;
-            const int sl = it % FT_RING;
-            float* const R1 = sm + FT_OFF_UR + (0 * FT_RING + sl) * FT_UPL + 4 * uq;
-            float* const R2 = sm + FT_OFF_UR + (1 * FT_RING + sl) * FT_UPL + 4 * uq;
-            float* const R3 = sm + FT_OFF_UR + (2 * FT_RING + sl) * FT_UPL + 4 * uq;
+            const int sl = it % RING;
+            float* const R1 = sm + OFF_UR + (0 * RING + sl) * FT_UPL + 4 * uq;
+            float* const R2 = sm + OFF_UR + (1 * RING + sl) * FT_UPL + 4 * uq;
+            float* const R3 = sm + OFF_UR + (2 * RING + sl) * FT_UPL + 4 * uq;
             {   // ---- u1 at (x+1/2, y, z): D+x s11, D-y s12, D-z s13
                 const float4 c11 = ld4s(P11, uq);
+                if (tmw) tmem_st4(tms, c11);
                 const float2 l = ld2s(P11, 4 * uq - 2), rr = ld2s(P11, 4 * uq + 4);
                 const float4 ya = ld4s(P12, q - 20), yb = ld4s(P12, q - 10), yd = ld4s(P12, q + 10);
                 float4 t1 = dpx(l, c11, rr), t2 = d4(ya, yb, c12, yd), t3 = d4(w13a, w13b, w13c, f13);
@@ -648,7 +697,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                     if (pz >= 0) t3 = pml_fwd_m(pm[2], a.mvo[2], idx_z(a, x, y, pz), ZT(T_A_INT)[kk & (FT_ZRING - 1)], ZT(T_B_INT)[kk & (FT_ZRING - 1)], t3, wr1);
                 }
                 if (MODE == FM_ADJ && pml1) {
-                    const float* S = SC1 + 0 * FT_RING * FT_UPL;
+                    const float* S = SC1 + 0 * RING * FT_UPL;
                     if (exa == 0) t1 = t1 + dpx(ld2s(S, 4 * uq - 2), ld4s(S, uq), ld2s(S, 4 * uq + 4));
                     if (yex) t2 = t2 + d4(ld4s(S, uq - 20), ld4s(S, uq - 10), ld4s(S, uq), ld4s(S, uq + 10));
                     else if (neary) t2 = t2 + adj_y(a, a.mvi[10], a.mvo[10], YT(T_A_HALF), YT(T_B_HALF), x, y - 2, kk, 2, ya, yb, c12, yd, wr1 && exa != 1);
@@ -661,6 +710,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             {   // ---- u2 at (x, y+1/2, z): D-x s12, D+y s22, D-z s23
                 const float2 l = ld2s(P12, 4 * q - 2), rr = ld2s(P12, 4 * q + 4);
                 const float4 yb = ld4s(P22, q - 10), c22 = ld4s(P22, q), yc = ld4s(P22, q + 10), yd = ld4s(P22, q + 20);
+                if (tmw) tmem_st4(tms + 4u, c22);
                 float4 t1 = dmx(l, c12, rr), t2 = d4(yb, c22, yc, yd), t3 = d4(w23a, w23b, w23c, f23);
                 if (MODE == FM_FWD && pml1) {
                     if (colq >= 0) t1 = pml_fwd_m(pm[3], a.mvo[3], idx_x(a, colq, y, kk), tab4(XT(T_A_INT), x), tab4(XT(T_B_INT), x), t1, wr1);
@@ -668,7 +718,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                     if (pz >= 0) t3 = pml_fwd_m(pm[5], a.mvo[5], idx_z(a, x, y, pz), ZT(T_A_INT)[kk & (FT_ZRING - 1)], ZT(T_B_INT)[kk & (FT_ZRING - 1)], t3, wr1);
                 }
                 if (MODE == FM_ADJ && pml1) {
-                    const float* S = SC1 + 1 * FT_RING * FT_UPL;
+                    const float* S = SC1 + 1 * RING * FT_UPL;
                     if (exa == 0) t1 = t1 + dmx(ld2s(S, 4 * uq - 2), ld4s(S, uq), ld2s(S, 4 * uq + 4));
                     if (yex) t2 = t2 + d4(ld4s(S, uq - 10), ld4s(S, uq), ld4s(S, uq + 10), ld4s(S, uq + 20));
                     else if (neary) t2 = t2 + adj_y(a, a.mvi[13], a.mvo[13], YT(T_A_INT), YT(T_B_INT), x, y - 1, kk, 1, yb, c22, yc, yd, wr1 && exa != 1);
@@ -687,7 +737,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                     if (pz >= 0) t3 = pml_fwd_m(pm[8], a.mvo[8], idx_z(a, x, y, pz), ZT(T_A_HALF)[kk & (FT_ZRING - 1)], ZT(T_B_HALF)[kk & (FT_ZRING - 1)], t3, wr1);
                 }
                 if (MODE == FM_ADJ && pml1) {
-                    const float* S = SC1 + 2 * FT_RING * FT_UPL;
+                    const float* S = SC1 + 2 * RING * FT_UPL;
                     if (exa == 0) t1 = t1 + dmx(ld2s(S, 4 * uq - 2), ld4s(S, uq), ld2s(S, 4 * uq + 4));
                     if (yex) t2 = t2 + d4(ld4s(S, uq - 20), ld4s(S, uq - 10), ld4s(S, uq), ld4s(S, uq + 10));
                     else if (neary) t2 = t2 + adj_y(a, a.mvi[16], a.mvo[16], YT(T_A_HALF), YT(T_B_HALF), x, y - 2, kk, 2, ya, yb, w23c, yd, wr1 && exa != 1);
@@ -742,9 +792,10 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                 ldg4_into(e2[0], a.mvi[exa] + i2, se2); ldg4_into(e2[1], a.mvi[3 + exa] + i2, se2); ldg4_into(e2[2], a.mvi[6 + exa] + i2, se2);
             }
         }
+        if (tmw) tmem_wait_st();
         if (pml && tid >= 360 && tid < 364) {   // z table ring: plane kk + 3 (first read after the barrier)
             const int t = tid - 360, z = kk + 3;
-            sm[FT_OFF_ZT + t * FT_ZRING + (z & (FT_ZRING - 1))] = (unsigned)z < (unsigned)a.nz ? __ldg(a.tab[2][t] + z) : 0.0f;
+            sm[OFF_ZT + t * FT_ZRING + (z & (FT_ZRING - 1))] = (unsigned)z < (unsigned)a.nz ? __ldg(a.tab[2][t] + z) : 0.0f;
         }
         __syncthreads();
         // every thread is past stage 1 of `it` and stage 2 of `it - 1`: refill the slots they freed
@@ -758,14 +809,9 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             kE = fE != 0 && fE == fMu;                                     // rho, alpha slot (it + 3) % 3 holds plane it (>= 0)
             kMu = it >= 3 && fMu != 0 && fMu == fM3;
             kLam = it >= 2 && fLam != 0 && fLam == fM3;
-            if (it + 1 < itn) issueU(it + 1);   // needed first ; slot of plane it - 3: its last cross-thread reads were in stage 2 of it - 1
-#ifdef FT_EXP_PFU
-            if (it + FT_EXP_PFU < itn) {
-                tma_prefetch_plane(&tmS36, cx40, cy36, cz0 + it + FT_EXP_PFU, U1);
-                tma_prefetch_plane(&tmS36, cx40, cy36, cz0 + it + FT_EXP_PFU, U2);
-                tma_prefetch_plane(&tmS36, cx40, cy36, cz0 + it + FT_EXP_PFU, U3);
-            }
-#endif
+            // needed first ; ring of 4: slot of plane it - 3, whose last cross-thread reads were in stage 2 of it - 1 (ring of 5:
+            // plane it + 2 into the slot of plane it - 3 likewise)
+            if (it + ULEAD < itn) issueU(it + ULEAD);
             if (it + 2 <= itn) issueM(it, fMu, fLam, kMu, kLam);
             if (exa < 0 && it + 2 < itn) issueG(it + 2, fE, 0u, kE);   // exchange CTAs: after stage 2 (its slots are their scratch)
         }
@@ -776,10 +822,10 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
         // that the first stage 2, at it = 4, finds u(ks-1) and u3(ks-2) in registers)
         float4 cc1 = z4, cc2 = z4, cc3 = z4;
         if (inner && it >= 2) {
-            const int pc = ((it + 2) % FT_RING) * FT_UPL;      // slot of plane it - 2
-            cc1 = ld4s(sm + FT_OFF_UR + 0 * FT_RING * FT_UPL + pc, uq);
-            cc2 = ld4s(sm + FT_OFF_UR + 1 * FT_RING * FT_UPL + pc, uq);
-            cc3 = ld4s(sm + FT_OFF_UR + 2 * FT_RING * FT_UPL + pc, uq);
+            const int pc = ((it + RING - 2) % RING) * FT_UPL;      // slot of plane it - 2
+            cc1 = ld4s(sm + OFF_UR + 0 * RING * FT_UPL + pc, uq);
+            cc2 = ld4s(sm + OFF_UR + 1 * RING * FT_UPL + pc, uq);
+            cc3 = ld4s(sm + OFF_UR + 2 * RING * FT_UPL + pc, uq);
         }
         // Adjoint slab CTAs: Y = a T' of the own quad (T' = b T'_old + u_bar(ks), not stored here: stage 1 of plane ks did)
         // for the three terms of the exchange axis, into the s22 / s12 / s11 planes that stage 1 has finished with.
@@ -790,10 +836,10 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             if (act1 && it >= 4) {
                 float4 Y0 = z4, Y1 = z4, Y2 = z4;
                 if (pok && (unsigned)ks < (unsigned)a.nz) {
-                    const int pc = ((it + 2) % FT_RING) * FT_UPL;      // slot of the centre plane it - 2
-                    const float4 v1 = ld4s(sm + FT_OFF_UR + 0 * FT_RING * FT_UPL + pc, uq);
-                    const float4 v2 = ld4s(sm + FT_OFF_UR + 1 * FT_RING * FT_UPL + pc, uq);
-                    const float4 v3 = ld4s(sm + FT_OFF_UR + 2 * FT_RING * FT_UPL + pc, uq);
+                    const int pc = ((it + RING - 2) % RING) * FT_UPL;      // slot of the centre plane it - 2
+                    const float4 v1 = ld4s(sm + OFF_UR + 0 * RING * FT_UPL + pc, uq);
+                    const float4 v2 = ld4s(sm + OFF_UR + 1 * RING * FT_UPL + pc, uq);
+                    const float4 v3 = ld4s(sm + OFF_UR + 2 * RING * FT_UPL + pc, uq);
                     if (exa == 0) {
                         const float4 ai = tab4(XT(T_A_INT), x), bi = tab4(XT(T_B_INT), x);
                         Y0 = adj_own_x(e2[0], a.mvo[0], i2, se2, tab4(XT(T_A_HALF), x), tab4(XT(T_B_HALF), x), v1, inner);
@@ -813,17 +859,29 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             }
             __syncthreads();
         }
+        // SOM 2: the old s11, s22, s12 of plane ks, parked by this thread in stage 1 two iterations ago (warp-wide
+        // instructions, hence outside the divergent block below)
+        float4 so11 = z4, so22 = z4, so12 = z4;
+        if (tmw && it >= 4) {
+            const uint32_t tml = tm0 + (uint32_t)((it + 1) % 3) * 12u;     // plane it - 2
+            so11 = tmem_ld4(tml); so22 = tmem_ld4(tml + 4u); so12 = tmem_ld4(tml + 8u);
+            tmem_wait_ld();
+        }
         if (inner && it >= 4) {
             const int j = it - 2;             // relative plane of ks
-            // old s12(ks): the one own-column load left on the LSU path (an L2 hit: group ks fetched the plane two
+            // SOM 0, 1: old s12(ks) (and s11, s22) by own-column loads (L2 hits: group ks fetched the planes two
             // iterations ago).  Issued here and consumed at the end of the stage: a load in flight across the loop
             // back-edge makes ptxas wait for it at the loop head, every iteration.
-            const float4 so12 = ldg4(in + S12 * box + (long long)ks * a.sz + gxy);
-            const float* U1p = sm + FT_OFF_UR + 0 * FT_RING * FT_UPL;
-            const float* U2p = sm + FT_OFF_UR + 1 * FT_RING * FT_UPL;
-            const float* U3p = sm + FT_OFF_UR + 2 * FT_RING * FT_UPL;
-            const int p0 = (j % FT_RING) * FT_UPL;
-            const int pp1 = ((j + 1) % FT_RING) * FT_UPL, pp2 = ((j + 2) % FT_RING) * FT_UPL;
+            if (SOM != 2) so12 = ldg4(in + S12 * box + (long long)ks * a.sz + gxy);
+            if (SOM == 1) {
+                so11 = ldg4(in + S11 * box + (long long)ks * a.sz + gxy);
+                so22 = ldg4(in + S22 * box + (long long)ks * a.sz + gxy);
+            }
+            const float* U1p = sm + OFF_UR + 0 * RING * FT_UPL;
+            const float* U2p = sm + OFF_UR + 1 * RING * FT_UPL;
+            const float* U3p = sm + OFF_UR + 2 * RING * FT_UPL;
+            const int p0 = (j % RING) * FT_UPL;
+            const int pp1 = ((j + 1) % RING) * FT_UPL, pp2 = ((j + 2) % RING) * FT_UPL;
             const int pz = pml ? yzslab_row(ks, a.nz, a.P) : -1;
             const bool bz = pml && (ks - 2 < a.P || ks + 2 >= a.nz - 1 - a.P);
             const bool pml2 = bx || by || bz;       // inner threads have storage: 0 <= x < nx, 0 <= y < ny, zb <= ks < ze
@@ -896,8 +954,12 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             const float4 lam = ld4s(sm + FT_OFF_LAM + (it & 1) * FT_LPL, (r - 2) * 8 + (qx - 1));   // lambda(ks), by TMA
             const float4 ldiv = (kL * lam) * (e11 + e22 + e33);
             const int lq = (r - 2) * 8 + (qx - 1);
-            const float4 n11 = ld4s(sm + FT_OFF_SO + (2 * (it & 1) + 0) * FT_LPL, lq) + fma4(mn2, e11, ldiv);
-            const float4 n22 = ld4s(sm + FT_OFF_SO + (2 * (it & 1) + 1) * FT_LPL, lq) + fma4(mn2, e22, ldiv);
+            if (SOM == 0) {
+                so11 = ld4s(sm + FT_OFF_SO + (2 * (it & 1) + 0) * FT_LPL, lq);
+                so22 = ld4s(sm + FT_OFF_SO + (2 * (it & 1) + 1) * FT_LPL, lq);
+            }
+            const float4 n11 = so11 + fma4(mn2, e11, ldiv);
+            const float4 n22 = so22 + fma4(mn2, e22, ldiv);
             const float4 n33 = w33a + fma4(mn2, e33, ldiv);
             const float4 n12 = fma4(mxy, g12 + g21, so12);
             const float4 n13 = fma4(mxz, g13 + g31, w13a);
@@ -935,22 +997,38 @@ k_step(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUtens
        const __grid_constant__ CUtensorMap tmL, const __grid_constant__ CUtensorMap tmS32, const FusedArgs a)
 {
     extern __shared__ __align__(1024) float sm[];
-    int* s_next = reinterpret_cast<int*>(sm + FT_OFF_ZT + 4 * FT_ZRING);
+    constexpr int SOM = FT_SOM(MODE);
+    int* s_next = reinterpret_cast<int*>(sm + FusedMap<SOM>::OFF_TICKET);
     const int n = a.work_end - a.work_begin;
     bool first = true;
+    uint32_t tmem_base = 0;
+    if (SOM == 2) {      // tensor memory for the parked old stresses: allocated once per (persistent) CTA by warp 0
+        uint32_t* s_tm = reinterpret_cast<uint32_t*>(s_next + 1);
+        if (threadIdx.x < 32) {
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(s_tm)), "r"(FT_TMEM_COLS) : "memory");
+            asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+        }
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        tmem_base = *s_tm;
+    }
     for (;;) {
         if (threadIdx.x == 0) *s_next = (int)atomicAdd(a.queue, 1u);
         __syncthreads();                 // also: every thread is done with the previous brick's shared memory
         const int b = *s_next;
         if (b >= n) break;
         const int4 wk = __ldg(a.work + a.work_begin + b);
-        if (MODE != FM_PLAIN && (wk.x & FT_WORK_SLAB)) fused_brick<MODE, true>(sm, tmS40, tmS36, tmM37, tmM36, tmL, tmS32, a, wk, first);
-        else if (wk.x & FT_WORK_NOEDGE) fused_brick<FM_PLAIN, false>(sm, tmS40, tmS36, tmM37, tmM36, tmL, tmS32, a, wk, first);
-        else fused_brick<FM_PLAIN, true>(sm, tmS40, tmS36, tmM37, tmM36, tmL, tmS32, a, wk, first);
+        if (MODE != FM_PLAIN && (wk.x & FT_WORK_SLAB)) fused_brick<MODE, true, SOM>(sm, tmS40, tmS36, tmM37, tmM36, tmL, tmS32, a, wk, first, tmem_base);
+        else if (wk.x & FT_WORK_NOEDGE) fused_brick<FM_PLAIN, false, SOM>(sm, tmS40, tmS36, tmM37, tmM36, tmL, tmS32, a, wk, first, tmem_base);
+        else fused_brick<FM_PLAIN, true, SOM>(sm, tmS40, tmS36, tmM37, tmM36, tmL, tmS32, a, wk, first, tmem_base);
         first = false;
         // generic-proxy writes of this brick (tables, exchange planes) precede the TMA writes of the next one
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads();                 // *s_next is read by all before thread 0 overwrites it
+    }
+    if (SOM == 2 && threadIdx.x < 32) {   // (every thread left its last brick through the loop's __syncthreads)
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(FT_TMEM_COLS) : "memory");
     }
     if (threadIdx.x == 0) {
         __threadfence();

@@ -725,26 +725,27 @@ static void fused_step(pact_ctx* c, Launcher& ln, int cur, float sgn, int kind)
     fa.mflag = c->elide ? c->d_mflag : nullptr;
     for (int k = 0; k < 18; ++k) { fa.mvi[k] = c->mvbuf[cur][k]; fa.mvo[k] = c->mvbuf[1 - cur][k]; }
     cudaStream_t st = c->stream;
-    auto launch = [&](int b0, int b1) {
+    // plain: the range holds no C-PML brick, so the kernel without C-PML code (and its register budget) serves it
+    auto launch = [&](int b0, int b1, bool plain) {
         if (b1 <= b0) return;
         fa.work_begin = b0; fa.work_end = b1;
         const int grid = std::min(c->num_sms, b1 - b0);
         if (use_acoustic(c)) {      // mu = 0 everywhere: one stress field, 44 B per cell-step (kernels_acoustic.cuh)
-            if (fa.P == 0) k_step_acoustic<FM_PLAIN><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmL, c->tmS32[cur], fa);
+            if (fa.P == 0 || plain) k_step_acoustic<FM_PLAIN><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmL, c->tmS32[cur], fa);
             else if (sgn > 0.0f) k_step_acoustic<FM_FWD><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmL, c->tmS32[cur], fa);
             else k_step_acoustic<FM_ADJ><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmL, c->tmS32[cur], fa);
         }
-        else if (fa.P == 0) k_step<FM_PLAIN><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fa);
+        else if (fa.P == 0 || plain) k_step<FM_PLAIN><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fa);
         else if (sgn > 0.0f) k_step<FM_FWD><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fa);
         else k_step<FM_ADJ><<<grid, FT_NT, FT_SMEM_BYTES, st>>>(c->tmS40[cur], c->tmS36[cur], c->tmM37, c->tmM36, c->tmL, c->tmS32[cur], fa);
     };
     if (!c->split_launch || c->nslab == 0 || c->nslab == c->nwork) {
-        ln.run(kind, [&] { launch(0, c->nwork); });
+        ln.run(kind, [&] { launch(0, c->nwork, c->nslab == 0); });
         return;
     }
     const int k_slab = sgn > 0.0f ? PACT_K_FWD_SLAB : PACT_K_ADJ_SLAB, k_int = sgn > 0.0f ? PACT_K_FWD_INTERIOR : PACT_K_ADJ_INTERIOR;
-    ln.run(k_slab, [&] { launch(0, c->nslab); });
-    ln.run(k_int, [&] { launch(c->nslab, c->nwork); });
+    ln.run(k_slab, [&] { launch(0, c->nslab, false); });
+    ln.run(k_int, [&] { launch(c->nslab, c->nwork, true); });
 }
 
 // Eq. 58 right to left: tau, then for m = 0..M-1 { Theta ; W' unless m = M-1 }
