@@ -56,6 +56,12 @@
 // iteration earlier.
 // The mode is a property of the kernel (template parameter SOM of the brick routine, FusedMap below).
 #define FT_RING 4                     // mode 0: u planes in the ring: ks .. ks+2 and the slot u_old(kk+1) is landing in
+// C-PML memory variables stream from HBM and are used right after they are requested: each thread asks for the record
+// it will load FT_PFMV planes later to be brought into L2 (measured at 512^3: 2 planes ahead -2 % forward, -5 % adjoint
+// slab launch; 1, 3, 4 planes ahead and L1 prefetches did not pay)
+#ifndef FT_PFMV
+#define FT_PFMV 2
+#endif
 #define FT_TMEM_COLS 128              // tensor-memory columns allocated per CTA (mode 2): 3 warps per lane quarter x 36
 
 // shared memory map (floats).  Planes are only as tall as their readers need: s11, s13 (x neighbours only) and
@@ -131,8 +137,13 @@ struct FusedArgs {
     int xl, xr, wx;        // x slab: columns [0,xl) and [xr, nxq) ; wx = xl + nxq - xr ; quad aligned
     int nxq;               // nx rounded up to a multiple of 4
     int wyz;               // slab width along y and z: 2P+1
-    const float* mvi[18];  // memory variables read:  phi[3a+b] = [0..9), psi[3a+b] = [9..18)
+    const float* mvi[18];  // memory variables read:  phi[3a+b] = [0..9), psi[3a+b] = [9..18)   (fluid-only kernels)
     float* mvo[18];        // memory variables written
+    // The elastic kernels see the same storage as six groups g = 3 * kind + b (kind 0: phi, 1: psi ; b = slab axis), the
+    // three components a of a quad interleaved: float offset 3 * o + 4 * a, o = the quad's offset in the layout above.
+    // One address per axis and stage then serves three loads and three stores (immediate offsets 0, 16, 32 bytes).
+    const float* mgi[6];
+    float* mgo[6];
 };
 
 // ---- PTX wrappers: mbarrier + TMA (SASS: SYNCS.*, UTMALDG) --------------------------------------
@@ -264,6 +275,11 @@ __device__ __forceinline__ void ldg4_into(float4& v, const float* p, bool pred)
         "}"
         : "+f"(v.x), "+f"(v.y), "+f"(v.z), "+f"(v.w)
         : "l"(p), "r"((int)pred));
+}
+// request the line at p into L2 (no register, no scoreboard)
+__device__ __forceinline__ void prefetch_l2(const float* p, bool pred)
+{
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %1, 0;\n\t@p prefetch.global.L2 [%0];\n\t}" ::"l"(p), "r"((int)pred) : "memory");
 }
 __device__ __forceinline__ void stg4(float* p, float4 v) { *reinterpret_cast<float4*>(p) = v; }
 
@@ -399,6 +415,83 @@ __device__ __forceinline__ float4 adj_own_x(float4 Told, float* To, long long i,
     if (wr) stg4(To + i, Tn);
     return a4 * Tn;
 }
+// ---- the same pieces on the interleaved layout (FusedArgs::mgi / mgo) with 32-bit float offsets --------------------
+// Forward recursion, branch-free: outside the slab a = 0 and the old value is 0, so m = 0 and t is returned unchanged.
+// `mo` points at the quad's record (component offset included).
+__device__ __forceinline__ float4 pml_fwd_p(float4 m_old, float* mo, float4 a4, float4 b4, float4 t, bool wr)
+{
+    const float4 m = fma4(b4, m_old, a4 * t);
+    if (wr) stg4(mo, m);
+    return t + m;
+}
+__device__ __forceinline__ float4 pml_fwd_p(float4 m_old, float* mo, float a1, float b1, float4 t, bool wr)
+{
+    const float4 m = fma4(b1, m_old, a1 * t);
+    if (wr) stg4(mo, m);
+    return t + m;
+}
+// X along y: rows r0..r0+3 ; obase = float offset of (row 0 of the y slab, own x) on the plane ; rs = floats per slab row
+__device__ __forceinline__ float4 adj_y3(const FusedArgs& a, const float* __restrict__ Ti, float* __restrict__ To,
+                                         const float* __restrict__ ta, const float* __restrict__ tb,
+                                         int obase, int rs, int r0, int own, float4 s0, float4 s1, float4 s2, float4 s3, bool wr)
+{
+    const float4 s[4] = {s0, s1, s2, s3};
+    float4 T[4];
+    int i[4];
+    bool in[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int p = yzslab_row(r0 + k, a.ny, a.P);
+        in[k] = p >= 0;
+        i[k] = in[k] ? obase + p * rs : 0;
+        T[k] = f4(0.0f);
+        ldg4_into(T[k], Ti + i[k], in[k]);
+    }
+    float4 X[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const float bk = in[k] ? tb[r0 + k] : 0.0f, ak = in[k] ? ta[r0 + k] : 0.0f;
+        const float4 Tn = fma4(bk, T[k], s[k]);
+        if (wr && k == own && in[k]) stg4(To + i[k], Tn);
+        X[k] = ak * Tn;
+    }
+    return d4(X[0], X[1], X[2], X[3]);
+}
+// X along z: planes z0..z0+3 ; oq = float offset of the own quad on slab row 0 ; rs = floats per slab row (plane)
+__device__ __forceinline__ float4 adj_z3(const FusedArgs& a, const float* __restrict__ Ti, float* __restrict__ To,
+                                         const float* __restrict__ ta, const float* __restrict__ tb,
+                                         int oq, int rs, int z0, int own, float4 s0, float4 s1, float4 s2, float4 s3, bool wr)
+{
+    const float4 s[4] = {s0, s1, s2, s3};
+    float4 T[4];
+    int i[4];
+    bool in[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int p = yzslab_row(z0 + k, a.nz, a.P);
+        in[k] = p >= 0;
+        i[k] = in[k] ? oq + p * rs : 0;
+        T[k] = f4(0.0f);
+        ldg4_into(T[k], Ti + i[k], in[k]);
+    }
+    float4 X[4];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const float bk = tb[(z0 + k) & (FT_ZRING - 1)], ak = in[k] ? ta[(z0 + k) & (FT_ZRING - 1)] : 0.0f;
+        const float4 Tn = fma4(bk, T[k], s[k]);
+        if (wr && k == own && in[k]) stg4(To + i[k], Tn);
+        X[k] = ak * Tn;
+    }
+    return d4(X[0], X[1], X[2], X[3]);
+}
+// own quad, old T already in registers ; `To` points at the quad's record
+__device__ __forceinline__ float4 adj_own_p(float4 Told, float* To, bool in_slab, float4 a4, float4 b4, float4 s, bool wr)
+{
+    if (!in_slab) return f4(0.0f);
+    const float4 Tn = fma4(b4, Told, s);
+    if (wr) stg4(To, Tn);
+    return a4 * Tn;
+}
 // =================================================================================================
 // The fused step.  MODE selects the C-PML code carried by the launch (FM_*); see DESIGN.md for the
 // index algebra.  Relative plane j <-> z = zb - 2 + j ; iteration `it` computes u(kk = zb - 2 + it)
@@ -459,6 +552,15 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
     // adjoint: slab axis whose filtered taps this CTA exchanges through shared memory (x if it touches the x slabs,
     // else y), -1 = none.  CTA-uniform: it adds block barriers.
     const int exa = (MODE == FM_ADJ) ? (bx ? 0 : (by ? 1 : -1)) : -1;
+    // Memory variables (interleaved layout): running float offsets of the own quad's record at plane kk in the x and y
+    // slabs, of row 0 of the y slab (adjoint taps), and the plane-independent part in the z slabs.  32 bits suffice
+    // (pact_create checks) and one add per plane replaces the 64-bit index products.
+    const bool hx = pok && colq >= 0, hy = pok && prow >= 0;
+    const int sxp = 3 * a.ny * a.wx, syp = 3 * a.wyz * a.nxq, szp = 3 * a.ny * a.nxq, rsy = 3 * a.nxq;
+    int ox = hx ? 3 * (((zb - 2) * a.ny + y) * a.wx + colq) : 0;
+    int oy = hy ? 3 * (((zb - 2) * a.wyz + prow) * a.nxq + x) : 0;
+    int oyb = pok ? 3 * ((zb - 2) * a.wyz * a.nxq + x) : 0;
+    const int ozq = pok ? 3 * (y * a.nxq + x) : 0;
 
     const float* in = a.in;
     const long long box = a.box;
@@ -595,27 +697,37 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
 #pragma unroll
             for (int k = 0; k < 9; ++k) pm[k] = f4(0.0f);
             if (bx || by || (pml && (kk - 2 < a.P || kk + 2 >= a.nz - 1 - a.P))) {
-                const bool ok = pok && (unsigned)kk < (unsigned)a.nz;
-                const int pzk = ok ? yzslab_row(kk, a.nz, a.P) : -1;
-                const bool ex = ok && colq >= 0, ey = ok && prow >= 0, ez = pzk >= 0;
-                const long long ix = ex ? idx_x(a, colq, y, kk) : 0, iy = ey ? idx_y(a, x, prow, kk) : 0, iz = ez ? idx_z(a, x, y, pzk) : 0;
-                ldg4_into(pm[0], a.mvi[0] + ix, ex); ldg4_into(pm[3], a.mvi[3] + ix, ex); ldg4_into(pm[6], a.mvi[6] + ix, ex);
-                ldg4_into(pm[1], a.mvi[1] + iy, ey); ldg4_into(pm[4], a.mvi[4] + iy, ey); ldg4_into(pm[7], a.mvi[7] + iy, ey);
-                ldg4_into(pm[2], a.mvi[2] + iz, ez); ldg4_into(pm[5], a.mvi[5] + iz, ez); ldg4_into(pm[8], a.mvi[8] + iz, ez);
+                const bool zok = (unsigned)kk < (unsigned)a.nz;
+                const int pzk = zok ? yzslab_row(kk, a.nz, a.P) : -1;          // CTA-uniform
+                const bool ex = hx && zok, ey = hy && zok, ez = pok && pzk >= 0;
+                const float* gx = a.mgi[0] + ox;
+                const float* gy = a.mgi[1] + oy;
+                const float* gz = a.mgi[2] + (ez ? ozq + pzk * szp : 0);
+                if (bx) { ldg4_into(pm[0], gx, ex); ldg4_into(pm[3], gx + 4, ex); ldg4_into(pm[6], gx + 8, ex); }
+                if (by) { ldg4_into(pm[1], gy, ey); ldg4_into(pm[4], gy + 4, ey); ldg4_into(pm[7], gy + 8, ey); }
+                if (pzk >= 0) { ldg4_into(pm[2], gz, ez); ldg4_into(pm[5], gz + 4, ez); ldg4_into(pm[8], gz + 8, ez); }
+#if FT_PFMV > 0
+                const bool zpf = kk + FT_PFMV < a.nz;
+                if (bx) prefetch_l2(gx + FT_PFMV * sxp, ex && zpf);
+                if (by) prefetch_l2(gy + FT_PFMV * syp, ey && zpf);
+#endif
             }
         }
         // adjoint exchange CTAs: the three old T of the own quad (plane kk) for the pre-block of stage 1, issued ahead
         float4 e1[3];
-        long long ie1 = 0;
+        int oe1 = 0;
         bool se1 = false;
         if (MODE == FM_ADJ) {
             e1[0] = e1[1] = e1[2] = f4(0.0f);
             if (exa >= 0) {
                 const bool ok = pok && (unsigned)kk < (unsigned)a.nz;
                 se1 = ok && (exa == 0 ? colq >= 0 : prow >= 0);
-                ie1 = se1 ? (exa == 0 ? idx_x(a, colq, y, kk) : idx_y(a, x, prow, kk)) : 0;
-                const int k0 = 9 + exa;
-                ldg4_into(e1[0], a.mvi[k0] + ie1, se1); ldg4_into(e1[1], a.mvi[k0 + 3] + ie1, se1); ldg4_into(e1[2], a.mvi[k0 + 6] + ie1, se1);
+                oe1 = se1 ? (exa == 0 ? ox : oy) : 0;
+                const float* ge = a.mgi[3 + exa] + oe1;
+                ldg4_into(e1[0], ge, se1); ldg4_into(e1[1], ge + 4, se1); ldg4_into(e1[2], ge + 8, se1);
+#if FT_PFMV > 0
+                prefetch_l2(ge + FT_PFMV * (exa == 0 ? sxp : syp), se1 && kk + FT_PFMV < a.nz);
+#endif
             }
         }
         mbar_wait(&barG[it & 1], (it >> 1) & 1);
@@ -637,15 +749,15 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                     if (exa == 0) {
                         const float4 o11 = ld4s(sm + FT_OFF_S11 + (it & 1) * FT_UPL, uq);
                         const float4 ai = tab4(XT(T_A_INT), x), bi = tab4(XT(T_B_INT), x), ah = tab4(XT(T_A_HALF), x), bh = tab4(XT(T_B_HALF), x);
-                        X0 = adj_own_x(e1[0], a.mvo[9], ie1, se1, ai, bi, o11, wr);
-                        X1 = adj_own_x(e1[1], a.mvo[12], ie1, se1, ah, bh, o12, wr);
-                        X2 = adj_own_x(e1[2], a.mvo[15], ie1, se1, ah, bh, w13c, wr);
+                        X0 = adj_own_p(e1[0], a.mgo[3] + oe1, se1, ai, bi, o11, wr);
+                        X1 = adj_own_p(e1[1], a.mgo[3] + oe1 + 4, se1, ah, bh, o12, wr);
+                        X2 = adj_own_p(e1[2], a.mgo[3] + oe1 + 8, se1, ah, bh, w13c, wr);
                     } else {
                         const float4 o22 = ld4s(sm + FT_OFF_S22 + (it & 1) * FT_BOX, q);
                         const float4 ai = f4(YT(T_A_INT)[y]), bi = f4(YT(T_B_INT)[y]), ah = f4(YT(T_A_HALF)[y]), bh = f4(YT(T_B_HALF)[y]);
-                        X0 = adj_own_x(e1[0], a.mvo[10], ie1, se1, ah, bh, o12, wr);
-                        X1 = adj_own_x(e1[1], a.mvo[13], ie1, se1, ai, bi, o22, wr);
-                        X2 = adj_own_x(e1[2], a.mvo[16], ie1, se1, ah, bh, w23c, wr);
+                        X0 = adj_own_p(e1[0], a.mgo[4] + oe1, se1, ah, bh, o12, wr);
+                        X1 = adj_own_p(e1[1], a.mgo[4] + oe1 + 4, se1, ai, bi, o22, wr);
+                        X2 = adj_own_p(e1[2], a.mgo[4] + oe1 + 8, se1, ah, bh, w23c, wr);
                     }
                 }
                 *reinterpret_cast<float4*>(SC1 + 0 * RING * FT_UPL + 4 * uq) = X0;
@@ -672,7 +784,9 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             // C-PML at this plane: z slab position of kk ; is any tap of the thread inside a slab
             const int pz = (pml && zin) ? yzslab_row(kk, a.nz, a.P) : -1;
             const bool bz = pml && (kk - 2 < a.P || kk + 2 >= a.nz - 1 - a.P);
-            const bool pml1 = (bx || by || bz) && pok && zin;
+            const bool slab1 = bx || by || bz;                       // CTA-uniform
+            const bool pml1 = slab1 && pok && zin;
+            const int oz1 = ozq + (pz >= 0 ? pz : 0) * szp;          // z-slab record of the own quad at plane kk
 
             // staggered coefficients (reading G10): J = 1 - dt alpha_b, B = dt/(h rho_b)
             const float4 r0 = ld4s(PR, uq), a0 = ld4s(PA, uq);
@@ -691,17 +805,17 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                 const float2 l = ld2s(P11, 4 * uq - 2), rr = ld2s(P11, 4 * uq + 4);
                 const float4 ya = ld4s(P12, q - 20), yb = ld4s(P12, q - 10), yd = ld4s(P12, q + 10);
                 float4 t1 = dpx(l, c11, rr), t2 = d4(ya, yb, c12, yd), t3 = d4(w13a, w13b, w13c, f13);
-                if (MODE == FM_FWD && pml1) {
-                    if (colq >= 0) t1 = pml_fwd_m(pm[0], a.mvo[0], idx_x(a, colq, y, kk), tab4(XT(T_A_HALF), x), tab4(XT(T_B_HALF), x), t1, wr1);
-                    if (prow >= 0) t2 = pml_fwd_m(pm[1], a.mvo[1], idx_y(a, x, prow, kk), YT(T_A_INT)[y], YT(T_B_INT)[y], t2, wr1);
-                    if (pz >= 0) t3 = pml_fwd_m(pm[2], a.mvo[2], idx_z(a, x, y, pz), ZT(T_A_INT)[kk & (FT_ZRING - 1)], ZT(T_B_INT)[kk & (FT_ZRING - 1)], t3, wr1);
+                if (MODE == FM_FWD && slab1) {
+                    if (bx) t1 = pml_fwd_p(pm[0], a.mgo[0] + ox, tab4(XT(T_A_HALF), x), tab4(XT(T_B_HALF), x), t1, wr1 && hx);
+                    if (by) t2 = pml_fwd_p(pm[1], a.mgo[1] + oy, YT(T_A_INT)[y], YT(T_B_INT)[y], t2, wr1 && hy);
+                    if (pz >= 0) t3 = pml_fwd_p(pm[2], a.mgo[2] + oz1, ZT(T_A_INT)[kk & (FT_ZRING - 1)], ZT(T_B_INT)[kk & (FT_ZRING - 1)], t3, wr1);
                 }
                 if (MODE == FM_ADJ && pml1) {
                     const float* S = SC1 + 0 * RING * FT_UPL;
                     if (exa == 0) t1 = t1 + dpx(ld2s(S, 4 * uq - 2), ld4s(S, uq), ld2s(S, 4 * uq + 4));
                     if (yex) t2 = t2 + d4(ld4s(S, uq - 20), ld4s(S, uq - 10), ld4s(S, uq), ld4s(S, uq + 10));
-                    else if (neary) t2 = t2 + adj_y(a, a.mvi[10], a.mvo[10], YT(T_A_HALF), YT(T_B_HALF), x, y - 2, kk, 2, ya, yb, c12, yd, wr1 && exa != 1);
-                    if (bz) t3 = t3 + adj_z(a, a.mvi[11], a.mvo[11], ZT(T_A_HALF), ZT(T_B_HALF), x, y, kk - 2, 2, w13a, w13b, w13c, f13, wr1);
+                    else if (neary) t2 = t2 + adj_y3(a, a.mgi[4], a.mgo[4], YT(T_A_HALF), YT(T_B_HALF), oyb, rsy, y - 2, 2, ya, yb, c12, yd, wr1 && exa != 1);
+                    if (bz) t3 = t3 + adj_z3(a, a.mgi[5], a.mgo[5], ZT(T_A_HALF), ZT(T_B_HALF), ozq, szp, kk - 2, 2, w13a, w13b, w13c, f13, wr1);
                 }
                 const float4 rxp = shl1(r0, PR[4 * uq + 4]), axp = shl1(a0, PA[4 * uq + 4]);
                 mbar_wait(&barU[it & 1], (it >> 1) & 1);      // u_old(kk) has landed in the ring slot
@@ -712,17 +826,17 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                 const float4 yb = ld4s(P22, q - 10), c22 = ld4s(P22, q), yc = ld4s(P22, q + 10), yd = ld4s(P22, q + 20);
                 if (tmw) tmem_st4(tms + 4u, c22);
                 float4 t1 = dmx(l, c12, rr), t2 = d4(yb, c22, yc, yd), t3 = d4(w23a, w23b, w23c, f23);
-                if (MODE == FM_FWD && pml1) {
-                    if (colq >= 0) t1 = pml_fwd_m(pm[3], a.mvo[3], idx_x(a, colq, y, kk), tab4(XT(T_A_INT), x), tab4(XT(T_B_INT), x), t1, wr1);
-                    if (prow >= 0) t2 = pml_fwd_m(pm[4], a.mvo[4], idx_y(a, x, prow, kk), YT(T_A_HALF)[y], YT(T_B_HALF)[y], t2, wr1);
-                    if (pz >= 0) t3 = pml_fwd_m(pm[5], a.mvo[5], idx_z(a, x, y, pz), ZT(T_A_INT)[kk & (FT_ZRING - 1)], ZT(T_B_INT)[kk & (FT_ZRING - 1)], t3, wr1);
+                if (MODE == FM_FWD && slab1) {
+                    if (bx) t1 = pml_fwd_p(pm[3], a.mgo[0] + ox + 4, tab4(XT(T_A_INT), x), tab4(XT(T_B_INT), x), t1, wr1 && hx);
+                    if (by) t2 = pml_fwd_p(pm[4], a.mgo[1] + oy + 4, YT(T_A_HALF)[y], YT(T_B_HALF)[y], t2, wr1 && hy);
+                    if (pz >= 0) t3 = pml_fwd_p(pm[5], a.mgo[2] + oz1 + 4, ZT(T_A_INT)[kk & (FT_ZRING - 1)], ZT(T_B_INT)[kk & (FT_ZRING - 1)], t3, wr1);
                 }
                 if (MODE == FM_ADJ && pml1) {
                     const float* S = SC1 + 1 * RING * FT_UPL;
                     if (exa == 0) t1 = t1 + dmx(ld2s(S, 4 * uq - 2), ld4s(S, uq), ld2s(S, 4 * uq + 4));
                     if (yex) t2 = t2 + d4(ld4s(S, uq - 10), ld4s(S, uq), ld4s(S, uq + 10), ld4s(S, uq + 20));
-                    else if (neary) t2 = t2 + adj_y(a, a.mvi[13], a.mvo[13], YT(T_A_INT), YT(T_B_INT), x, y - 1, kk, 1, yb, c22, yc, yd, wr1 && exa != 1);
-                    if (bz) t3 = t3 + adj_z(a, a.mvi[14], a.mvo[14], ZT(T_A_HALF), ZT(T_B_HALF), x, y, kk - 2, 2, w23a, w23b, w23c, f23, wr1);
+                    else if (neary) t2 = t2 + adj_y3(a, a.mgi[4] + 4, a.mgo[4] + 4, YT(T_A_INT), YT(T_B_INT), oyb, rsy, y - 1, 1, yb, c22, yc, yd, wr1 && exa != 1);
+                    if (bz) t3 = t3 + adj_z3(a, a.mgi[5] + 4, a.mgo[5] + 4, ZT(T_A_HALF), ZT(T_B_HALF), ozq, szp, kk - 2, 2, w23a, w23b, w23c, f23, wr1);
                 }
                 const float4 ryp = ld4s(PR, uq + 10), ayp = ld4s(PA, uq + 10);
                 n2 = fma4(fma4(mh, a0 + ayp, one), *reinterpret_cast<const float4*>(R2), (kB * rcp4(r0 + ryp)) * (t1 + t2 + t3));
@@ -731,17 +845,17 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                 const float2 l = ld2s(P13, 4 * uq - 2), rr = ld2s(P13, 4 * uq + 4);
                 const float4 ya = ld4s(P23, q - 20), yb = ld4s(P23, q - 10), yd = ld4s(P23, q + 10);
                 float4 t1 = dmx(l, w13c, rr), t2 = d4(ya, yb, w23c, yd), t3 = d4(w33b, w33c, w33d, f33);
-                if (MODE == FM_FWD && pml1) {
-                    if (colq >= 0) t1 = pml_fwd_m(pm[6], a.mvo[6], idx_x(a, colq, y, kk), tab4(XT(T_A_INT), x), tab4(XT(T_B_INT), x), t1, wr1);
-                    if (prow >= 0) t2 = pml_fwd_m(pm[7], a.mvo[7], idx_y(a, x, prow, kk), YT(T_A_INT)[y], YT(T_B_INT)[y], t2, wr1);
-                    if (pz >= 0) t3 = pml_fwd_m(pm[8], a.mvo[8], idx_z(a, x, y, pz), ZT(T_A_HALF)[kk & (FT_ZRING - 1)], ZT(T_B_HALF)[kk & (FT_ZRING - 1)], t3, wr1);
+                if (MODE == FM_FWD && slab1) {
+                    if (bx) t1 = pml_fwd_p(pm[6], a.mgo[0] + ox + 8, tab4(XT(T_A_INT), x), tab4(XT(T_B_INT), x), t1, wr1 && hx);
+                    if (by) t2 = pml_fwd_p(pm[7], a.mgo[1] + oy + 8, YT(T_A_INT)[y], YT(T_B_INT)[y], t2, wr1 && hy);
+                    if (pz >= 0) t3 = pml_fwd_p(pm[8], a.mgo[2] + oz1 + 8, ZT(T_A_HALF)[kk & (FT_ZRING - 1)], ZT(T_B_HALF)[kk & (FT_ZRING - 1)], t3, wr1);
                 }
                 if (MODE == FM_ADJ && pml1) {
                     const float* S = SC1 + 2 * RING * FT_UPL;
                     if (exa == 0) t1 = t1 + dmx(ld2s(S, 4 * uq - 2), ld4s(S, uq), ld2s(S, 4 * uq + 4));
                     if (yex) t2 = t2 + d4(ld4s(S, uq - 20), ld4s(S, uq - 10), ld4s(S, uq), ld4s(S, uq + 10));
-                    else if (neary) t2 = t2 + adj_y(a, a.mvi[16], a.mvo[16], YT(T_A_HALF), YT(T_B_HALF), x, y - 2, kk, 2, ya, yb, w23c, yd, wr1 && exa != 1);
-                    if (bz) t3 = t3 + adj_z(a, a.mvi[17], a.mvo[17], ZT(T_A_INT), ZT(T_B_INT), x, y, kk - 1, 1, w33b, w33c, w33d, f33, wr1);
+                    else if (neary) t2 = t2 + adj_y3(a, a.mgi[4] + 8, a.mgo[4] + 8, YT(T_A_HALF), YT(T_B_HALF), oyb, rsy, y - 2, 2, ya, yb, w23c, yd, wr1 && exa != 1);
+                    if (bz) t3 = t3 + adj_z3(a, a.mgi[5] + 8, a.mgo[5] + 8, ZT(T_A_INT), ZT(T_B_INT), ozq, szp, kk - 1, 1, w33b, w33c, w33d, f33, wr1);
                 }
                 const float4 rzp = ld4s(Rbase + s3n * FT_RPL, uq), azp = ld4s(Abase + s3n * FT_RPL, uq);
                 n3 = fma4(fma4(mh, a0 + azp, one), *reinterpret_cast<const float4*>(R3), (kB * rcp4(r0 + rzp)) * (t1 + t2 + t3));
@@ -771,25 +885,36 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             for (int k = 0; k < 9; ++k) qm[k] = f4(0.0f);
             if (bx || by || (pml && (kk - 4 < a.P || kk >= a.nz - 1 - a.P))) {
                 const bool ok = inner && it >= 4;
-                const int pzk = ok ? yzslab_row(kk - 2, a.nz, a.P) : -1;
-                const bool ex = ok && colq >= 0, ey = ok && prow >= 0, ez = pzk >= 0;
-                const long long ix = ex ? idx_x(a, colq, y, kk - 2) : 0, iy = ey ? idx_y(a, x, prow, kk - 2) : 0, iz = ez ? idx_z(a, x, y, pzk) : 0;
-                ldg4_into(qm[0], a.mvi[9] + ix, ex); ldg4_into(qm[3], a.mvi[12] + ix, ex); ldg4_into(qm[6], a.mvi[15] + ix, ex);
-                ldg4_into(qm[1], a.mvi[10] + iy, ey); ldg4_into(qm[4], a.mvi[13] + iy, ey); ldg4_into(qm[7], a.mvi[16] + iy, ey);
-                ldg4_into(qm[2], a.mvi[11] + iz, ez); ldg4_into(qm[5], a.mvi[14] + iz, ez); ldg4_into(qm[8], a.mvi[17] + iz, ez);
+                const int pzk = it >= 4 ? yzslab_row(kk - 2, a.nz, a.P) : -1;      // CTA-uniform
+                const bool ex = ok && colq >= 0, ey = ok && prow >= 0, ez = ok && pzk >= 0;
+                const float* gx = a.mgi[3] + (ox - 2 * sxp);
+                const float* gy = a.mgi[4] + (oy - 2 * syp);
+                const float* gz = a.mgi[5] + (ez ? ozq + pzk * szp : 0);
+                if (bx) { ldg4_into(qm[0], gx, ex); ldg4_into(qm[3], gx + 4, ex); ldg4_into(qm[6], gx + 8, ex); }
+                if (by) { ldg4_into(qm[1], gy, ey); ldg4_into(qm[4], gy + 4, ey); ldg4_into(qm[7], gy + 8, ey); }
+                if (pzk >= 0) { ldg4_into(qm[2], gz, ez); ldg4_into(qm[5], gz + 4, ez); ldg4_into(qm[8], gz + 8, ez); }
+#if FT_PFMV > 0
+                const bool zpf = kk - 2 + FT_PFMV < a.nz;
+                if (bx) prefetch_l2(gx + FT_PFMV * sxp, ex && zpf);
+                if (by) prefetch_l2(gy + FT_PFMV * syp, ey && zpf);
+#endif
             }
         }
         // adjoint exchange CTAs: the three old T' of the own quad (plane ks = kk - 2) for the pre-block of stage 2
         float4 e2[3];
-        long long i2 = 0;
+        int oe2 = 0;
         bool se2 = false;
         if (MODE == FM_ADJ) {
             e2[0] = e2[1] = e2[2] = f4(0.0f);
             if (exa >= 0 && it >= 4) {
                 const bool ok = pok && (unsigned)(kk - 2) < (unsigned)a.nz;
                 se2 = ok && (exa == 0 ? colq >= 0 : prow >= 0);
-                i2 = se2 ? (exa == 0 ? idx_x(a, colq, y, kk - 2) : idx_y(a, x, prow, kk - 2)) : 0;
-                ldg4_into(e2[0], a.mvi[exa] + i2, se2); ldg4_into(e2[1], a.mvi[3 + exa] + i2, se2); ldg4_into(e2[2], a.mvi[6 + exa] + i2, se2);
+                oe2 = se2 ? (exa == 0 ? ox - 2 * sxp : oy - 2 * syp) : 0;
+                const float* ge = a.mgi[exa] + oe2;
+                ldg4_into(e2[0], ge, se2); ldg4_into(e2[1], ge + 4, se2); ldg4_into(e2[2], ge + 8, se2);
+#if FT_PFMV > 0
+                prefetch_l2(ge + FT_PFMV * (exa == 0 ? sxp : syp), se2 && kk - 2 + FT_PFMV < a.nz);
+#endif
             }
         }
         if (tmw) tmem_wait_st();
@@ -842,14 +967,14 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                     const float4 v3 = ld4s(sm + OFF_UR + 2 * RING * FT_UPL + pc, uq);
                     if (exa == 0) {
                         const float4 ai = tab4(XT(T_A_INT), x), bi = tab4(XT(T_B_INT), x);
-                        Y0 = adj_own_x(e2[0], a.mvo[0], i2, se2, tab4(XT(T_A_HALF), x), tab4(XT(T_B_HALF), x), v1, inner);
-                        Y1 = adj_own_x(e2[1], a.mvo[3], i2, se2, ai, bi, v2, inner);
-                        Y2 = adj_own_x(e2[2], a.mvo[6], i2, se2, ai, bi, v3, inner);
+                        Y0 = adj_own_p(e2[0], a.mgo[0] + oe2, se2, tab4(XT(T_A_HALF), x), tab4(XT(T_B_HALF), x), v1, inner);
+                        Y1 = adj_own_p(e2[1], a.mgo[0] + oe2 + 4, se2, ai, bi, v2, inner);
+                        Y2 = adj_own_p(e2[2], a.mgo[0] + oe2 + 8, se2, ai, bi, v3, inner);
                     } else {
                         const float4 ai = f4(YT(T_A_INT)[y]), bi = f4(YT(T_B_INT)[y]);
-                        Y0 = adj_own_x(e2[0], a.mvo[1], i2, se2, ai, bi, v1, inner);
-                        Y1 = adj_own_x(e2[1], a.mvo[4], i2, se2, f4(YT(T_A_HALF)[y]), f4(YT(T_B_HALF)[y]), v2, inner);
-                        Y2 = adj_own_x(e2[2], a.mvo[7], i2, se2, ai, bi, v3, inner);
+                        Y0 = adj_own_p(e2[0], a.mgo[1] + oe2, se2, ai, bi, v1, inner);
+                        Y1 = adj_own_p(e2[1], a.mgo[1] + oe2 + 4, se2, f4(YT(T_A_HALF)[y]), f4(YT(T_B_HALF)[y]), v2, inner);
+                        Y2 = adj_own_p(e2[2], a.mgo[1] + oe2 + 8, se2, ai, bi, v3, inner);
                     }
                 }
                 *reinterpret_cast<float4*>(SC2a + 4 * uq) = Y0;
@@ -885,6 +1010,8 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             const int pz = pml ? yzslab_row(ks, a.nz, a.P) : -1;
             const bool bz = pml && (ks - 2 < a.P || ks + 2 >= a.nz - 1 - a.P);
             const bool pml2 = bx || by || bz;       // inner threads have storage: 0 <= x < nx, 0 <= y < ny, zb <= ks < ze
+            const int ox2 = ox - 2 * sxp, oy2 = oy - 2 * syp, oyb2 = oyb - 2 * syp;      // plane ks
+            const int oz2 = ozq + (pz >= 0 ? pz : 0) * szp;
             float4 e11, e22, e33, g12, g21, g13, g31, g23, g32;
             {   // ---- derivatives of u1: D-x (e11), D+y (g12), D+z (g13)
                 const float4 c = cc1;
@@ -893,15 +1020,15 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                 const float4 za = u1m1, zc = ld4s(U1p + pp1, uq), zd = ld4s(U1p + pp2, uq);
                 e11 = dmx(l, c, rr); g12 = d4(ya, c, yc, yd); g13 = d4(za, c, zc, zd);
                 if (MODE == FM_FWD && pml2) {
-                    if (colq >= 0) e11 = pml_fwd_m(qm[0], a.mvo[9], idx_x(a, colq, y, ks), tab4(XT(T_A_INT), x), tab4(XT(T_B_INT), x), e11, true);
-                    if (prow >= 0) g12 = pml_fwd_m(qm[1], a.mvo[10], idx_y(a, x, prow, ks), YT(T_A_HALF)[y], YT(T_B_HALF)[y], g12, true);
-                    if (pz >= 0) g13 = pml_fwd_m(qm[2], a.mvo[11], idx_z(a, x, y, pz), ZT(T_A_HALF)[ks & (FT_ZRING - 1)], ZT(T_B_HALF)[ks & (FT_ZRING - 1)], g13, true);
+                    if (bx) e11 = pml_fwd_p(qm[0], a.mgo[3] + ox2, tab4(XT(T_A_INT), x), tab4(XT(T_B_INT), x), e11, colq >= 0);
+                    if (by) g12 = pml_fwd_p(qm[1], a.mgo[4] + oy2, YT(T_A_HALF)[y], YT(T_B_HALF)[y], g12, prow >= 0);
+                    if (pz >= 0) g13 = pml_fwd_p(qm[2], a.mgo[5] + oz2, ZT(T_A_HALF)[ks & (FT_ZRING - 1)], ZT(T_B_HALF)[ks & (FT_ZRING - 1)], g13, true);
                 }
                 if (MODE == FM_ADJ && pml2) {
                     if (exa == 0) e11 = e11 + dmx(ld2s(SC2a, 4 * uq - 2), ld4s(SC2a, uq), ld2s(SC2a, 4 * uq + 4));
                     if (exa == 1) g12 = g12 + d4(ld4s(SC2a, uq - 10), ld4s(SC2a, uq), ld4s(SC2a, uq + 10), ld4s(SC2a, uq + 20));
-                    else if (neary) g12 = g12 + adj_y(a, a.mvi[1], a.mvo[1], YT(T_A_INT), YT(T_B_INT), x, y - 1, ks, 1, ya, c, yc, yd, true);
-                    if (bz) g13 = g13 + adj_z(a, a.mvi[2], a.mvo[2], ZT(T_A_INT), ZT(T_B_INT), x, y, ks - 1, 1, za, c, zc, zd, true);
+                    else if (neary) g12 = g12 + adj_y3(a, a.mgi[1], a.mgo[1], YT(T_A_INT), YT(T_B_INT), oyb2, rsy, y - 1, 1, ya, c, yc, yd, true);
+                    if (bz) g13 = g13 + adj_z3(a, a.mgi[2], a.mgo[2], ZT(T_A_INT), ZT(T_B_INT), ozq, szp, ks - 1, 1, za, c, zc, zd, true);
                 }
             }
             {   // ---- derivatives of u2: D+x (g21), D-y (e22), D+z (g23)
@@ -911,15 +1038,15 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                 const float4 za = u2m1, zc = ld4s(U2p + pp1, uq), zd = ld4s(U2p + pp2, uq);
                 g21 = dpx(l, c, rr); e22 = d4(ya, yb, c, yd); g23 = d4(za, c, zc, zd);
                 if (MODE == FM_FWD && pml2) {
-                    if (colq >= 0) g21 = pml_fwd_m(qm[3], a.mvo[12], idx_x(a, colq, y, ks), tab4(XT(T_A_HALF), x), tab4(XT(T_B_HALF), x), g21, true);
-                    if (prow >= 0) e22 = pml_fwd_m(qm[4], a.mvo[13], idx_y(a, x, prow, ks), YT(T_A_INT)[y], YT(T_B_INT)[y], e22, true);
-                    if (pz >= 0) g23 = pml_fwd_m(qm[5], a.mvo[14], idx_z(a, x, y, pz), ZT(T_A_HALF)[ks & (FT_ZRING - 1)], ZT(T_B_HALF)[ks & (FT_ZRING - 1)], g23, true);
+                    if (bx) g21 = pml_fwd_p(qm[3], a.mgo[3] + ox2 + 4, tab4(XT(T_A_HALF), x), tab4(XT(T_B_HALF), x), g21, colq >= 0);
+                    if (by) e22 = pml_fwd_p(qm[4], a.mgo[4] + oy2 + 4, YT(T_A_INT)[y], YT(T_B_INT)[y], e22, prow >= 0);
+                    if (pz >= 0) g23 = pml_fwd_p(qm[5], a.mgo[5] + oz2 + 4, ZT(T_A_HALF)[ks & (FT_ZRING - 1)], ZT(T_B_HALF)[ks & (FT_ZRING - 1)], g23, true);
                 }
                 if (MODE == FM_ADJ && pml2) {
                     if (exa == 0) g21 = g21 + dpx(ld2s(SC2b, 4 * uq - 2), ld4s(SC2b, uq), ld2s(SC2b, 4 * uq + 4));
                     if (exa == 1) e22 = e22 + d4(ld4s(SC2b, uq - 20), ld4s(SC2b, uq - 10), ld4s(SC2b, uq), ld4s(SC2b, uq + 10));
-                    else if (neary) e22 = e22 + adj_y(a, a.mvi[4], a.mvo[4], YT(T_A_HALF), YT(T_B_HALF), x, y - 2, ks, 2, ya, yb, c, yd, true);
-                    if (bz) g23 = g23 + adj_z(a, a.mvi[5], a.mvo[5], ZT(T_A_INT), ZT(T_B_INT), x, y, ks - 1, 1, za, c, zc, zd, true);
+                    else if (neary) e22 = e22 + adj_y3(a, a.mgi[1] + 4, a.mgo[1] + 4, YT(T_A_HALF), YT(T_B_HALF), oyb2, rsy, y - 2, 2, ya, yb, c, yd, true);
+                    if (bz) g23 = g23 + adj_z3(a, a.mgi[2] + 4, a.mgo[2] + 4, ZT(T_A_INT), ZT(T_B_INT), ozq, szp, ks - 1, 1, za, c, zc, zd, true);
                 }
             }
             {   // ---- derivatives of u3: D+x (g31), D+y (g32), D-z (e33)
@@ -929,15 +1056,15 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                 const float4 za = u3m2, zb_ = u3m1, zd = ld4s(U3p + pp1, uq);
                 g31 = dpx(l, c, rr); g32 = d4(ya, c, yc, yd); e33 = d4(za, zb_, c, zd);
                 if (MODE == FM_FWD && pml2) {
-                    if (colq >= 0) g31 = pml_fwd_m(qm[6], a.mvo[15], idx_x(a, colq, y, ks), tab4(XT(T_A_HALF), x), tab4(XT(T_B_HALF), x), g31, true);
-                    if (prow >= 0) g32 = pml_fwd_m(qm[7], a.mvo[16], idx_y(a, x, prow, ks), YT(T_A_HALF)[y], YT(T_B_HALF)[y], g32, true);
-                    if (pz >= 0) e33 = pml_fwd_m(qm[8], a.mvo[17], idx_z(a, x, y, pz), ZT(T_A_INT)[ks & (FT_ZRING - 1)], ZT(T_B_INT)[ks & (FT_ZRING - 1)], e33, true);
+                    if (bx) g31 = pml_fwd_p(qm[6], a.mgo[3] + ox2 + 8, tab4(XT(T_A_HALF), x), tab4(XT(T_B_HALF), x), g31, colq >= 0);
+                    if (by) g32 = pml_fwd_p(qm[7], a.mgo[4] + oy2 + 8, YT(T_A_HALF)[y], YT(T_B_HALF)[y], g32, prow >= 0);
+                    if (pz >= 0) e33 = pml_fwd_p(qm[8], a.mgo[5] + oz2 + 8, ZT(T_A_INT)[ks & (FT_ZRING - 1)], ZT(T_B_INT)[ks & (FT_ZRING - 1)], e33, true);
                 }
                 if (MODE == FM_ADJ && pml2) {
                     if (exa == 0) g31 = g31 + dpx(ld2s(SC2c, 4 * uq - 2), ld4s(SC2c, uq), ld2s(SC2c, 4 * uq + 4));
                     if (exa == 1) g32 = g32 + d4(ld4s(SC2c, uq - 10), ld4s(SC2c, uq), ld4s(SC2c, uq + 10), ld4s(SC2c, uq + 20));
-                    else if (neary) g32 = g32 + adj_y(a, a.mvi[7], a.mvo[7], YT(T_A_INT), YT(T_B_INT), x, y - 1, ks, 1, ya, c, yc, yd, true);
-                    if (bz) e33 = e33 + adj_z(a, a.mvi[8], a.mvo[8], ZT(T_A_HALF), ZT(T_B_HALF), x, y, ks - 2, 2, za, zb_, c, zd, true);
+                    else if (neary) g32 = g32 + adj_y3(a, a.mgi[1] + 8, a.mgo[1] + 8, YT(T_A_INT), YT(T_B_INT), oyb2, rsy, y - 1, 1, ya, c, yc, yd, true);
+                    if (bz) e33 = e33 + adj_z3(a, a.mgi[2] + 8, a.mgo[2] + 8, ZT(T_A_HALF), ZT(T_B_HALF), ozq, szp, ks - 2, 2, za, zb_, c, zd, true);
                 }
             }
 
@@ -977,6 +1104,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             if (tid == FT_PROD && it + 2 < itn) issueG(it + 2, fE, 0u, kE);
         }
         u3m2 = u3m1; u1m1 = cc1; u2m1 = cc2; u3m1 = cc3;
+        if (MODE != FM_PLAIN) { ox += sxp; oy += syp; oyb += syp; }
         // slide the z windows
         w13a = w13b; w13b = w13c; w13c = f13;
         w23a = w23b; w23b = w23c; w23c = f23;

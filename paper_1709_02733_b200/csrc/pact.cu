@@ -85,6 +85,7 @@ struct pact_ctx {
     unsigned int* d_queue;   // [2] ticket counter + exit counter of the persistent launch
     int split_launch;        // diagnostic option: slab bricks and interior bricks as two launches, timed apart
     float* mvbuf[2][18];     // fused memory variables, two sets (read / written alternate every step)
+    float* mgbuf[2][6];      // the same storage as the elastic kernels see it: six groups of three interleaved components
     // host-buffer variants and pact_pgd / pact_power_iteration (gradient and residual)
     float* d_vol;            // [N]
     float* d_dat;            // [nt][L]
@@ -586,6 +587,11 @@ static int ensure_fused(pact_ctx* c)
         mv[2] = (long long)fa.nxq * g.ny * fa.wyz;
     }
     auto r32 = [](long long v) { return (v + 31) / 32 * 32; };
+    for (int b = 0; b < 3; ++b)     // the kernels index a group with 32-bit float offsets
+        if (3 * r32(mv[b]) + 64 > 0x7fffffffLL) {
+            snprintf(g_cuda_err, sizeof(g_cuda_err), "C-PML slab of axis %d too large for the fused kernels' 32-bit offsets", b);
+            return PACT_EINVAL;
+        }
     long long total = c->box * NFIELD;
     for (int b = 0; b < 3; ++b) total += 2 * 6 * r32(mv[b]);
     c->stateB_bytes = total * (long long)sizeof(float);
@@ -597,7 +603,11 @@ static int ensure_fused(pact_ctx* c)
     {
         float* p = c->stateB_base + c->box * NFIELD;
         for (int set = 0; set < 2; ++set)            // [0]: read at even steps, [1]: read at odd steps
+        {
+            float* q = p;       // elastic view (FusedArgs::mgi): group g = 3 * kind + axis, 3 * r32(mv[axis]) floats each
+            for (int gk = 0; gk < 6; ++gk) { c->mgbuf[set][gk] = q; q += 3 * r32(mv[gk % 3]); }
             for (int k = 0; k < 18; ++k) { c->mvbuf[set][k] = p; p += r32(mv[k % 3]); }
+        }
     }
     void* fn = nullptr;
     cudaDriverEntryPointQueryResult qres;
@@ -724,6 +734,7 @@ static void fused_step(pact_ctx* c, Launcher& ln, int cur, float sgn, int kind)
     fa.work = c->d_work;
     fa.mflag = c->elide ? c->d_mflag : nullptr;
     for (int k = 0; k < 18; ++k) { fa.mvi[k] = c->mvbuf[cur][k]; fa.mvo[k] = c->mvbuf[1 - cur][k]; }
+    for (int k = 0; k < 6; ++k) { fa.mgi[k] = c->mgbuf[cur][k]; fa.mgo[k] = c->mgbuf[1 - cur][k]; }
     cudaStream_t st = c->stream;
     // plain: the range holds no C-PML brick, so the kernel without C-PML code (and its register budget) serves it
     auto launch = [&](int b0, int b1, bool plain) {
