@@ -62,6 +62,20 @@
 #ifndef FT_PFMV
 #define FT_PFMV 2
 #endif
+// Windows in tensor memory (WT): the z windows of s13, s23, s33 (10 quads per thread) live in tensor memory instead of
+// registers; every warp then executes stage 1 convergently (the 24 spare lanes of warp 11 compute on in-range
+// shared-memory garbage and store nothing), because tcgen05.ld / st are warp-wide instructions.
+// Measured at 512^3: C-PML kernels -14 % (adjoint) / -3 % (forward) and room for SO mode 2 there (-7 % / -2 % more) ; the
+// C-PML-free kernel +3.5 % (it has no register shortage to relieve), so only the C-PML kernels use it.
+#ifndef FT_WT_PML
+#define FT_WT_PML 1
+#endif
+#ifndef FT_WT_PLAIN
+#define FT_WT_PLAIN 0
+#endif
+#define FT_WT(MODE) ((MODE) == FM_PLAIN ? FT_WT_PLAIN : FT_WT_PML)
+#define FT_TM_WARP 100                // columns per warp: parked old stresses 36 | s13 ring 16 | s23 ring 16 | s33 ring 32
+#define FT_TMEM_COLS_X 512
 #define FT_TMEM_COLS 128              // tensor-memory columns allocated per CTA (mode 2): 3 warps per lane quarter x 36
 
 // shared memory map (floats).  Planes are only as tall as their readers need: s11, s13 (x neighbours only) and
@@ -99,9 +113,9 @@ struct FusedMap {
 };
 #define FT_SMEM_BYTES (FusedMap<2>::BYTES > FusedMap<0>::BYTES ? FusedMap<2>::BYTES : FusedMap<0>::BYTES)
 static_assert(FT_SMEM_BYTES <= 232448, "shared-memory map exceeds 227 KB");
-// SO mode of the kernel that carries C-PML mode MODE: the C-PML kernels are at the register limit already
+// SO mode of the kernel that carries C-PML mode MODE (the C-PML kernels need WT for mode 2: registers)
 #ifndef FT_SOM_PML
-#define FT_SOM_PML 0
+#define FT_SOM_PML 2
 #endif
 #ifndef FT_SOM_PLAIN
 #define FT_SOM_PLAIN 2
@@ -498,7 +512,7 @@ __device__ __forceinline__ float4 adj_own_p(float4 Told, float* To, bool in_slab
 // and sigma(ks = kk - 2).
 // EDGE = false: the host vouches (FT_WORK_NOEDGE) that nothing this brick touches sticks out of the grid, so the lane
 // masks, the in-grid tests of the stores and the z range tests are compiled out.
-template <int MODE, bool EDGE, int SOM>
+template <int MODE, bool EDGE, int SOM, bool WT>
 __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtensorMap& tmS40, const CUtensorMap& tmS36,
                                             const CUtensorMap& tmM37, const CUtensorMap& tmM36, const CUtensorMap& tmL,
                                             const CUtensorMap& tmS32, const FusedArgs& a, const int4 wk, const bool first,
@@ -525,8 +539,9 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
     const int uq = tid;                     // quad index in a 40x36 plane
     // SOM 2: the thread's tensor-memory scratch (lane = its lane in the warp's lane quarter ; 36 columns per warp:
     // [plane % 3][s11, s22, s12][4]).  Warp 11 holds no tile quad and takes no part (its u-region lanes diverge).
-    const bool tmw = SOM == 2 && tid < 352;
-    const uint32_t tm0 = tmem_base + ((uint32_t)((tid >> 5) & 3) << 21) + (uint32_t)(tid >> 7) * 36u;
+    const bool tmw = SOM == 2 && (WT || tid < 352);
+    const uint32_t tm0 = tmem_base + ((uint32_t)((tid >> 5) & 3) << 21) + (uint32_t)(tid >> 7) * (WT ? FT_TM_WARP : 36u);
+    const uint32_t tW13 = tm0 + 36u, tW23 = tm0 + 52u, tW33 = tm0 + 68u;      // WT: ring slots of 4 columns, plane j -> j & 3 (s33: j & 7)
     const int mq = (r - 2) * 9 + (qx - 1);  // quad index in a mu plane (inner threads)
     // own-column global loads are legal where the padded box has storage
     const bool ld_ok = act1 && (!EDGE || ((y + PACT_HALO_Y < a.ny + 2 * PACT_HALO_Y) && (x + 3 + PACT_HALO_X < (int)a.sy)));
@@ -672,6 +687,12 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
         w33b = ld_ok ? ldg4(in + S33 * box + g - a.sz) : z4;
         w33c = ld_ok ? ldg4(in + S33 * box + g) : z4;
         w33d = ld_ok ? ldg4(in + S33 * box + g + a.sz) : z4;
+        if (WT) {      // planes -2, -1, 0 (s33: and 1) of the rings
+            tmem_st4(tW13 + 8u, w13a); tmem_st4(tW13 + 12u, w13b); tmem_st4(tW13, w13c);
+            tmem_st4(tW23 + 8u, w23a); tmem_st4(tW23 + 12u, w23b); tmem_st4(tW23, w23c);
+            tmem_st4(tW33 + 24u, w33a); tmem_st4(tW33 + 28u, w33b); tmem_st4(tW33, w33c); tmem_st4(tW33 + 4u, w33d);
+            tmem_wait_st();
+        }
     }
 
     // coefficient scales: sign of the step and the 1/c2 of the unnormalised differences (d1)
@@ -741,7 +762,11 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
         // stage 2 was passed by every thread).
         float* const SC1 = sm + OFF_UR + ((it + ULEAD) % RING) * FT_UPL;     // + f * RING * FT_UPL
         if (exa >= 0) {
-            if (act1) {
+            if (WT) {
+                if (exa == 0) w13c = tmem_ld4(tW13 + 4u * (it & 3)); else w23c = tmem_ld4(tW23 + 4u * (it & 3));
+                tmem_wait_ld();
+            }
+            if (WT || act1) {
                 float4 X0 = z4, X1 = z4, X2 = z4;
                 if (pok && zin) {
                     const bool wr = inner && kk >= zb && kk < ze;
@@ -760,15 +785,17 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                         X2 = adj_own_p(e1[2], a.mgo[4] + oe1 + 8, se1, ah, bh, w23c, wr);
                     }
                 }
-                *reinterpret_cast<float4*>(SC1 + 0 * RING * FT_UPL + 4 * uq) = X0;
-                *reinterpret_cast<float4*>(SC1 + 1 * RING * FT_UPL + 4 * uq) = X1;
-                *reinterpret_cast<float4*>(SC1 + 2 * RING * FT_UPL + 4 * uq) = X2;
+                if (!WT || act1) {
+                    *reinterpret_cast<float4*>(SC1 + 0 * RING * FT_UPL + 4 * uq) = X0;
+                    *reinterpret_cast<float4*>(SC1 + 1 * RING * FT_UPL + 4 * uq) = X1;
+                    *reinterpret_cast<float4*>(SC1 + 2 * RING * FT_UPL + 4 * uq) = X2;
+                }
                 asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // TMA overwrites these planes later
             }
             __syncthreads();
         }
         const bool yex = exa == 1 && r >= 2 && r < 34;      // all four y taps of this thread lie in the exchanged region
-        if (act1) {
+        if (WT || act1) {
             const float* P11 = sm + FT_OFF_S11 + (it & 1) * FT_UPL;
             const float* P22 = sm + FT_OFF_S22 + (it & 1) * FT_BOX;
             const float* P12 = sm + FT_OFF_S12 + (it & 1) * FT_BOX;
@@ -779,6 +806,9 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             f13 = ld4s(sm + FT_OFF_S13 + s3n * FT_UPL, uq);
             f23 = ld4s(sm + FT_OFF_S23 + s3n * FT_BOX, q);
             f33 = ld4s(sm + FT_OFF_S33 + (it & 1) * FT_UPL, uq);   // plane kk+2
+            if (WT) {
+                tmem_st4(tW13 + 4u * ((it + 1) & 3), f13); tmem_st4(tW23 + 4u * ((it + 1) & 3), f23); tmem_st4(tW33 + 4u * ((it + 2) & 7), f33);
+            }
 
             const bool wr1 = inner && kk >= zb && kk < ze;          // this CTA owns u(x..x+3, y, kk)
             // C-PML at this plane: z slab position of kk ; is any tap of the thread inside a slab
@@ -804,6 +834,10 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                 if (tmw) tmem_st4(tms, c11);
                 const float2 l = ld2s(P11, 4 * uq - 2), rr = ld2s(P11, 4 * uq + 4);
                 const float4 ya = ld4s(P12, q - 20), yb = ld4s(P12, q - 10), yd = ld4s(P12, q + 10);
+                if (WT) {
+                    w13a = tmem_ld4(tW13 + 4u * ((it + 2) & 3)); w13b = tmem_ld4(tW13 + 4u * ((it + 3) & 3)); w13c = tmem_ld4(tW13 + 4u * (it & 3));
+                    tmem_wait_ld();
+                }
                 float4 t1 = dpx(l, c11, rr), t2 = d4(ya, yb, c12, yd), t3 = d4(w13a, w13b, w13c, f13);
                 if (MODE == FM_FWD && slab1) {
                     if (bx) t1 = pml_fwd_p(pm[0], a.mgo[0] + ox, tab4(XT(T_A_HALF), x), tab4(XT(T_B_HALF), x), t1, wr1 && hx);
@@ -825,6 +859,10 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                 const float2 l = ld2s(P12, 4 * q - 2), rr = ld2s(P12, 4 * q + 4);
                 const float4 yb = ld4s(P22, q - 10), c22 = ld4s(P22, q), yc = ld4s(P22, q + 10), yd = ld4s(P22, q + 20);
                 if (tmw) tmem_st4(tms + 4u, c22);
+                if (WT) {
+                    w23a = tmem_ld4(tW23 + 4u * ((it + 2) & 3)); w23b = tmem_ld4(tW23 + 4u * ((it + 3) & 3)); w23c = tmem_ld4(tW23 + 4u * (it & 3));
+                    tmem_wait_ld();
+                }
                 float4 t1 = dmx(l, c12, rr), t2 = d4(yb, c22, yc, yd), t3 = d4(w23a, w23b, w23c, f23);
                 if (MODE == FM_FWD && slab1) {
                     if (bx) t1 = pml_fwd_p(pm[3], a.mgo[0] + ox + 4, tab4(XT(T_A_INT), x), tab4(XT(T_B_INT), x), t1, wr1 && hx);
@@ -844,6 +882,10 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             {   // ---- u3 at (x, y, z+1/2): D-x s13, D-y s23, D+z s33
                 const float2 l = ld2s(P13, 4 * uq - 2), rr = ld2s(P13, 4 * uq + 4);
                 const float4 ya = ld4s(P23, q - 20), yb = ld4s(P23, q - 10), yd = ld4s(P23, q + 10);
+                if (WT) {
+                    w33b = tmem_ld4(tW33 + 4u * ((it + 7) & 7)); w33c = tmem_ld4(tW33 + 4u * (it & 7)); w33d = tmem_ld4(tW33 + 4u * ((it + 1) & 7));
+                    tmem_wait_ld();
+                }
                 float4 t1 = dmx(l, w13c, rr), t2 = d4(ya, yb, w23c, yd), t3 = d4(w33b, w33c, w33d, f33);
                 if (MODE == FM_FWD && slab1) {
                     if (bx) t1 = pml_fwd_p(pm[6], a.mgo[0] + ox + 8, tab4(XT(T_A_INT), x), tab4(XT(T_B_INT), x), t1, wr1 && hx);
@@ -866,9 +908,11 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                 if (!(zin && m2)) { n1.z = 0.0f; n2.z = 0.0f; n3.z = 0.0f; }
                 if (!(zin && m3)) { n1.w = 0.0f; n2.w = 0.0f; n3.w = 0.0f; }
             }
-            *reinterpret_cast<float4*>(R1) = n1;
-            *reinterpret_cast<float4*>(R2) = n2;
-            *reinterpret_cast<float4*>(R3) = n3;
+            if (!WT || act1) {
+                *reinterpret_cast<float4*>(R1) = n1;
+                *reinterpret_cast<float4*>(R2) = n2;
+                *reinterpret_cast<float4*>(R3) = n3;
+            }
             // generic-proxy writes to a slot that issueU refills through the async proxy four iterations later
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             const long long g = (long long)kk * a.sz + gxy;
@@ -917,7 +961,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
 #endif
             }
         }
-        if (tmw) tmem_wait_st();
+        if (WT || tmw) tmem_wait_st();
         if (pml && tid >= 360 && tid < 364) {   // z table ring: plane kk + 3 (first read after the barrier)
             const int t = tid - 360, z = kk + 3;
             sm[OFF_ZT + t * FT_ZRING + (z & (FT_ZRING - 1))] = (unsigned)z < (unsigned)a.nz ? __ldg(a.tab[2][t] + z) : 0.0f;
@@ -987,9 +1031,14 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
         // SOM 2: the old s11, s22, s12 of plane ks, parked by this thread in stage 1 two iterations ago (warp-wide
         // instructions, hence outside the divergent block below)
         float4 so11 = z4, so22 = z4, so12 = z4;
-        if (tmw && it >= 4) {
-            const uint32_t tml = tm0 + (uint32_t)((it + 1) % 3) * 12u;     // plane it - 2
-            so11 = tmem_ld4(tml); so22 = tmem_ld4(tml + 4u); so12 = tmem_ld4(tml + 8u);
+        if ((WT || tmw) && it >= 4) {
+            if (tmw) {
+                const uint32_t tml = tm0 + (uint32_t)((it + 1) % 3) * 12u;     // plane it - 2
+                so11 = tmem_ld4(tml); so22 = tmem_ld4(tml + 4u); so12 = tmem_ld4(tml + 8u);
+            }
+            if (WT) {   // old s13, s23, s33 of plane ks = the oldest window entries
+                w13a = tmem_ld4(tW13 + 4u * ((it + 2) & 3)); w23a = tmem_ld4(tW23 + 4u * ((it + 2) & 3)); w33a = tmem_ld4(tW33 + 4u * ((it + 6) & 7));
+            }
             tmem_wait_ld();
         }
         if (inner && it >= 4) {
@@ -1106,9 +1155,11 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
         u3m2 = u3m1; u1m1 = cc1; u2m1 = cc2; u3m1 = cc3;
         if (MODE != FM_PLAIN) { ox += sxp; oy += syp; oyb += syp; }
         // slide the z windows
-        w13a = w13b; w13b = w13c; w13c = f13;
-        w23a = w23b; w23b = w23c; w23c = f23;
-        w33a = w33b; w33b = w33c; w33c = w33d; w33d = f33;
+        if (!WT) {
+            w13a = w13b; w13b = w13c; w13c = f13;
+            w23a = w23b; w23b = w23c; w23c = f23;
+            w33a = w33b; w33b = w33c; w33c = w33d; w33d = f33;
+        }
     }
 }
 
@@ -1130,10 +1181,12 @@ k_step(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUtens
     const int n = a.work_end - a.work_begin;
     bool first = true;
     uint32_t tmem_base = 0;
-    if (SOM == 2) {      // tensor memory for the parked old stresses: allocated once per (persistent) CTA by warp 0
+    constexpr bool WT = FT_WT(MODE) != 0;
+    constexpr int TMC = WT ? FT_TMEM_COLS_X : FT_TMEM_COLS;
+    if (SOM == 2 || WT) {      // tensor memory (parked old stresses, z windows): allocated once per (persistent) CTA by warp 0
         uint32_t* s_tm = reinterpret_cast<uint32_t*>(s_next + 1);
         if (threadIdx.x < 32) {
-            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(s_tm)), "r"(FT_TMEM_COLS) : "memory");
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(s_tm)), "r"(TMC) : "memory");
             asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
         }
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -1147,16 +1200,16 @@ k_step(const __grid_constant__ CUtensorMap tmS40, const __grid_constant__ CUtens
         const int b = *s_next;
         if (b >= n) break;
         const int4 wk = __ldg(a.work + a.work_begin + b);
-        if (MODE != FM_PLAIN && (wk.x & FT_WORK_SLAB)) fused_brick<MODE, true, SOM>(sm, tmS40, tmS36, tmM37, tmM36, tmL, tmS32, a, wk, first, tmem_base);
-        else if (wk.x & FT_WORK_NOEDGE) fused_brick<FM_PLAIN, false, SOM>(sm, tmS40, tmS36, tmM37, tmM36, tmL, tmS32, a, wk, first, tmem_base);
-        else fused_brick<FM_PLAIN, true, SOM>(sm, tmS40, tmS36, tmM37, tmM36, tmL, tmS32, a, wk, first, tmem_base);
+        if (MODE != FM_PLAIN && (wk.x & FT_WORK_SLAB)) fused_brick<MODE, true, SOM, WT>(sm, tmS40, tmS36, tmM37, tmM36, tmL, tmS32, a, wk, first, tmem_base);
+        else if (wk.x & FT_WORK_NOEDGE) fused_brick<FM_PLAIN, false, SOM, WT>(sm, tmS40, tmS36, tmM37, tmM36, tmL, tmS32, a, wk, first, tmem_base);
+        else fused_brick<FM_PLAIN, true, SOM, WT>(sm, tmS40, tmS36, tmM37, tmM36, tmL, tmS32, a, wk, first, tmem_base);
         first = false;
         // generic-proxy writes of this brick (tables, exchange planes) precede the TMA writes of the next one
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads();                 // *s_next is read by all before thread 0 overwrites it
     }
-    if (SOM == 2 && threadIdx.x < 32) {   // (every thread left its last brick through the loop's __syncthreads)
-        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(FT_TMEM_COLS) : "memory");
+    if ((SOM == 2 || WT) && threadIdx.x < 32) {   // (every thread left its last brick through the loop's __syncthreads)
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(TMC) : "memory");
     }
     if (threadIdx.x == 0) {
         __threadfence();
