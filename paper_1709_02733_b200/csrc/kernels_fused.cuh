@@ -823,7 +823,6 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             const float4 one = f4(1.0f), mh = f4(-0.5f);
             const float4 c12 = ld4s(P12, q);
             const uint32_t tms = tm0 + (uint32_t)(it % 3) * 12u;      // SOM 2: this plane's parking columns
-            if (tmw) tmem_st4(tms + 8u, c12);
             float4 n1, n2, n3;
             const int sl = it % RING;
             float* const R1 = sm + OFF_UR + (0 * RING + sl) * FT_UPL + 4 * uq;
@@ -831,7 +830,6 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             float* const R3 = sm + OFF_UR + (2 * RING + sl) * FT_UPL + 4 * uq;
             {   // ---- u1 at (x+1/2, y, z): D+x s11, D-y s12, D-z s13
                 const float4 c11 = ld4s(P11, uq);
-                if (tmw) tmem_st4(tms, c11);
                 const float2 l = ld2s(P11, 4 * uq - 2), rr = ld2s(P11, 4 * uq + 4);
                 const float4 ya = ld4s(P12, q - 20), yb = ld4s(P12, q - 10), yd = ld4s(P12, q + 10);
                 if (WT) {
@@ -839,6 +837,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                     tmem_wait_ld();
                 }
                 float4 t1 = dpx(l, c11, rr), t2 = d4(ya, yb, c12, yd), t3 = d4(w13a, w13b, w13c, f13);
+                if (tmw) { tmem_st4(tms, c11); tmem_st4(tms + 8u, c12); }      // parked after their first use: no wait for the LDS here
                 if (MODE == FM_FWD && slab1) {
                     if (bx) t1 = pml_fwd_p(pm[0], a.mgo[0] + ox, tab4(XT(T_A_HALF), x), tab4(XT(T_B_HALF), x), t1, wr1 && hx);
                     if (by) t2 = pml_fwd_p(pm[1], a.mgo[1] + oy, YT(T_A_INT)[y], YT(T_B_INT)[y], t2, wr1 && hy);
@@ -858,12 +857,12 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             {   // ---- u2 at (x, y+1/2, z): D-x s12, D+y s22, D-z s23
                 const float2 l = ld2s(P12, 4 * q - 2), rr = ld2s(P12, 4 * q + 4);
                 const float4 yb = ld4s(P22, q - 10), c22 = ld4s(P22, q), yc = ld4s(P22, q + 10), yd = ld4s(P22, q + 20);
-                if (tmw) tmem_st4(tms + 4u, c22);
                 if (WT) {
                     w23a = tmem_ld4(tW23 + 4u * ((it + 2) & 3)); w23b = tmem_ld4(tW23 + 4u * ((it + 3) & 3)); w23c = tmem_ld4(tW23 + 4u * (it & 3));
                     tmem_wait_ld();
                 }
                 float4 t1 = dmx(l, c12, rr), t2 = d4(yb, c22, yc, yd), t3 = d4(w23a, w23b, w23c, f23);
+                if (tmw) tmem_st4(tms + 4u, c22);
                 if (MODE == FM_FWD && slab1) {
                     if (bx) t1 = pml_fwd_p(pm[3], a.mgo[0] + ox + 4, tab4(XT(T_A_INT), x), tab4(XT(T_B_INT), x), t1, wr1 && hx);
                     if (by) t2 = pml_fwd_p(pm[4], a.mgo[1] + oy + 4, YT(T_A_HALF)[y], YT(T_B_HALF)[y], t2, wr1 && hy);
@@ -961,6 +960,19 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
 #endif
             }
         }
+        // SOM 2: the old s11, s22, s12 of plane ks = kk - 2, parked by this thread in stage 1 two iterations ago ; WT: the
+        // oldest window entries.  Warp-wide instructions, hence outside the divergent block of stage 2 ; requested here, ahead
+        // of the block barrier, and waited for at the top of stage 2.
+        float4 so11 = z4, so22 = z4, so12 = z4;
+        if ((WT || tmw) && it >= 4) {
+            if (tmw) {
+                const uint32_t tml = tm0 + (uint32_t)((it + 1) % 3) * 12u;     // plane it - 2
+                so11 = tmem_ld4(tml); so22 = tmem_ld4(tml + 4u); so12 = tmem_ld4(tml + 8u);
+            }
+            if (WT) {   // old s13, s23, s33 of plane ks = the oldest window entries
+                w13a = tmem_ld4(tW13 + 4u * ((it + 2) & 3)); w23a = tmem_ld4(tW23 + 4u * ((it + 2) & 3)); w33a = tmem_ld4(tW33 + 4u * ((it + 6) & 7));
+            }
+        }
         if (WT || tmw) tmem_wait_st();
         if (pml && tid >= 360 && tid < 364) {   // z table ring: plane kk + 3 (first read after the barrier)
             const int t = tid - 360, z = kk + 3;
@@ -1028,19 +1040,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             }
             __syncthreads();
         }
-        // SOM 2: the old s11, s22, s12 of plane ks, parked by this thread in stage 1 two iterations ago (warp-wide
-        // instructions, hence outside the divergent block below)
-        float4 so11 = z4, so22 = z4, so12 = z4;
-        if ((WT || tmw) && it >= 4) {
-            if (tmw) {
-                const uint32_t tml = tm0 + (uint32_t)((it + 1) % 3) * 12u;     // plane it - 2
-                so11 = tmem_ld4(tml); so22 = tmem_ld4(tml + 4u); so12 = tmem_ld4(tml + 8u);
-            }
-            if (WT) {   // old s13, s23, s33 of plane ks = the oldest window entries
-                w13a = tmem_ld4(tW13 + 4u * ((it + 2) & 3)); w23a = tmem_ld4(tW23 + 4u * ((it + 2) & 3)); w33a = tmem_ld4(tW33 + 4u * ((it + 6) & 7));
-            }
-            tmem_wait_ld();
-        }
+        if ((WT || tmw) && it >= 4) tmem_wait_ld();      // (requested ahead of the block barrier)
         if (inner && it >= 4) {
             const int j = it - 2;             // relative plane of ks
             // SOM 0, 1: old s12(ks) (and s11, s22) by own-column loads (L2 hits: group ks fetched the planes two
