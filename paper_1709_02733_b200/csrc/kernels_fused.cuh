@@ -731,6 +731,8 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                 const bool zpf = kk + FT_PFMV < a.nz;
                 if (bx) prefetch_l2(gx + FT_PFMV * sxp, ex && zpf);
                 if (by) prefetch_l2(gy + FT_PFMV * syp, ey && zpf);
+                const int pzf = yzslab_row(kk + FT_PFMV, a.nz, a.P);
+                if (pzf >= 0) prefetch_l2(a.mgi[2] + (ozq + pzf * szp), pok);
 #endif
             }
         }
@@ -739,6 +741,13 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
         int oe1 = 0;
         bool se1 = false;
         if (MODE == FM_ADJ) {
+#if FT_PFMV > 0
+            if (pml) {      // z slabs: the newest planes the transposed recursions of stage 1 / stage 2 will tap, FT_PFMV iterations on
+                const int p1 = yzslab_row(kk + 2 + FT_PFMV, a.nz, a.P), p2 = yzslab_row(kk + FT_PFMV, a.nz, a.P);
+                if (p1 >= 0) prefetch_l2(a.mgi[5] + (ozq + p1 * szp), pok);
+                if (p2 >= 0) prefetch_l2(a.mgi[2] + (ozq + p2 * szp), pok);
+            }
+#endif
             e1[0] = e1[1] = e1[2] = f4(0.0f);
             if (exa >= 0) {
                 const bool ok = pok && (unsigned)kk < (unsigned)a.nz;
@@ -940,6 +949,8 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                 const bool zpf = kk - 2 + FT_PFMV < a.nz;
                 if (bx) prefetch_l2(gx + FT_PFMV * sxp, ex && zpf);
                 if (by) prefetch_l2(gy + FT_PFMV * syp, ey && zpf);
+                const int pzf = yzslab_row(kk - 2 + FT_PFMV, a.nz, a.P);
+                if (pzf >= 0) prefetch_l2(a.mgi[5] + (ozq + pzf * szp), ok);
 #endif
             }
         }
