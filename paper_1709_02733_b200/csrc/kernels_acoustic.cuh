@@ -36,7 +36,7 @@ static_assert(AC_OFF_SC2 + FT_BOX <= FT_OFF_END, "acoustic shared-memory map ove
 static_assert(AC_OFF_W % 32 == 0 && AC_OFF_RHO % 32 == 0 && AC_OFF_ALP % 32 == 0 && AC_OFF_LAM % 32 == 0 && AC_OFF_SO % 32 == 0 &&
               AC_OFF_UR % 32 == 0 && AC_OFF_SC1 % 32 == 0, "TMA destinations are 128-byte aligned");
 
-template <int MODE>
+template <int MODE, bool EDGE>
 __device__ __forceinline__ void acoustic_brick(float* __restrict__ sm, const CUtensorMap& tmS40, const CUtensorMap& tmS36,
                                                const CUtensorMap& tmM37, const CUtensorMap& tmL, const CUtensorMap& tmS32,
                                                const FusedArgs& a, const int4 wk, const bool first)
@@ -54,16 +54,16 @@ __device__ __forceinline__ void acoustic_brick(float* __restrict__ sm, const CUt
     const bool act1 = tid < 360;
     const int qx = tid % 10, r = tid / 10;
     const int x = x0 - 4 + 4 * qx, y = y0 - 2 + r;
-    const bool inner = act1 && qx >= 1 && qx <= 8 && r >= 2 && r < 34 && x < a.nx && y < a.ny;
+    const bool inner = act1 && qx >= 1 && qx <= 8 && r >= 2 && r < 34 && (!EDGE || (x < a.nx && y < a.ny));
     const int q = tid + 20;                 // quad index in the 40 x 40 stress plane
     const int uq = tid;                     // quad index in a 40 x 36 plane
     const int lq = (r - 2) * 8 + (qx - 1);  // quad index in a 32 x 32 plane (inner threads)
-    const bool ld_ok = act1 && (y + PACT_HALO_Y < a.ny + 2 * PACT_HALO_Y) && (x + 3 + PACT_HALO_X < (int)a.sy);
+    const bool ld_ok = act1 && (!EDGE || ((y + PACT_HALO_Y < a.ny + 2 * PACT_HALO_Y) && (x + 3 + PACT_HALO_X < (int)a.sy)));
     const long long gxy = (long long)y * a.sy + x;
     const bool yin = (unsigned)y < (unsigned)a.ny;
     const bool m0 = yin && (unsigned)x < (unsigned)a.nx, m1 = yin && (unsigned)(x + 1) < (unsigned)a.nx;
     const bool m2 = yin && (unsigned)(x + 2) < (unsigned)a.nx, m3 = yin && (unsigned)(x + 3) < (unsigned)a.nx;
-    const bool edge_xy = x0 == 0 || y0 == 0 || x0 + FT_TX + 4 > a.nx || y0 + FT_TY + 2 > a.ny;
+    const bool edge_xy = EDGE && (x0 == 0 || y0 == 0 || x0 + FT_TX + 4 > a.nx || y0 + FT_TY + 2 > a.ny);
 
     const bool pml = MODE != FM_PLAIN && a.P > 0;
     const bool bx = pml && (x0 - 8 < a.xl || x0 + FT_TX + 8 > a.xr);
@@ -73,6 +73,14 @@ __device__ __forceinline__ void acoustic_brick(float* __restrict__ sm, const CUt
     const int prow = pok ? yzslab_row(y, a.ny, a.P) : -1;
     const bool neary = pok && (y - 2 < a.P || y + 2 >= a.ny - 1 - a.P);
     const int exa = (MODE == FM_ADJ) ? (bx ? 0 : (by ? 1 : -1)) : -1;
+    // memory variables: 32-bit running offsets of the own quad at plane kk (x, y slabs), of row 0 of the y slab (adjoint
+    // taps) and the plane-independent part in the z slabs (one add per plane instead of 64-bit index products)
+    const bool hx = pok && colq >= 0, hy = pok && prow >= 0;
+    const int sxp = a.ny * a.wx, syp = a.wyz * a.nxq, szp = a.ny * a.nxq;
+    int ox = hx ? ((zb - 2) * a.ny + y) * a.wx + colq : 0;
+    int oy = hy ? ((zb - 2) * a.wyz + prow) * a.nxq + x : 0;
+    int oyb = pok ? (zb - 2) * a.wyz * a.nxq + x : 0;
+    const int ozq = pok ? y * a.nxq + x : 0;
 
     const float* in = a.in;
     const long long box = a.box;
@@ -177,9 +185,16 @@ __device__ __forceinline__ void acoustic_brick(float* __restrict__ sm, const CUt
                 const bool ok = pok && (unsigned)kk < (unsigned)a.nz;
                 const int pzk = ok ? yzslab_row(kk, a.nz, a.P) : -1;
                 const bool ex = ok && colq >= 0, ey = ok && prow >= 0, ez = pzk >= 0;
-                ldg4_into(pm0, a.mvi[0] + (ex ? idx_x(a, colq, y, kk) : 0), ex);
-                ldg4_into(pm1, a.mvi[4] + (ey ? idx_y(a, x, prow, kk) : 0), ey);
-                ldg4_into(pm2, a.mvi[8] + (ez ? idx_z(a, x, y, pzk) : 0), ez);
+                ldg4_into(pm0, a.mvi[0] + (ex ? ox : 0), ex);
+                ldg4_into(pm1, a.mvi[4] + (ey ? oy : 0), ey);
+                ldg4_into(pm2, a.mvi[8] + (ez ? ozq + pzk * szp : 0), ez);
+#if FT_PFMV > 0
+                const bool zpf = kk + FT_PFMV < a.nz;
+                prefetch_l2(a.mvi[0] + (ox + FT_PFMV * sxp), ex && zpf);
+                prefetch_l2(a.mvi[4] + (oy + FT_PFMV * syp), ey && zpf);
+                const int pzf = yzslab_row(kk + FT_PFMV, a.nz, a.P);
+                if (pzf >= 0) prefetch_l2(a.mvi[8] + (ozq + pzf * szp), pok);
+#endif
             }
         }
         // adjoint exchange CTAs: old T of psi_aa (a = exchange axis) of the own quad at plane kk
@@ -189,14 +204,14 @@ __device__ __forceinline__ void acoustic_brick(float* __restrict__ sm, const CUt
         if (MODE == FM_ADJ && exa >= 0) {
             const bool ok = pok && (unsigned)kk < (unsigned)a.nz;
             se1 = ok && (exa == 0 ? colq >= 0 : prow >= 0);
-            ie1 = se1 ? (exa == 0 ? idx_x(a, colq, y, kk) : idx_y(a, x, prow, kk)) : 0;
+            ie1 = se1 ? (exa == 0 ? ox : oy) : 0;
             ldg4_into(e1, a.mvi[9 + 4 * exa] + ie1, se1);
         }
         mbar_wait(&barG[it & 1], (it >> 1) & 1);
 
         const int s3 = it % 3, s3n = (it + 1) % 3;
         float4 f33 = z4;
-        const bool zin = (unsigned)kk < (unsigned)a.nz;
+        const bool zin = !EDGE || (unsigned)kk < (unsigned)a.nz;
         const float* PS = sm + AC_OFF_S + (it & 1) * FT_BOX;                          // s(kk), 40 x 40
         // ------------------------------------------------------------------ stage 1: u(kk)
         float* const SC1 = sm + AC_OFF_SC1;
@@ -234,7 +249,7 @@ __device__ __forceinline__ void acoustic_brick(float* __restrict__ sm, const CUt
             {   // ---- u1 at (x+1/2, y, z): D+x s
                 float4 t1 = dpx(ld2s(PS, 4 * q - 2), cs, ld2s(PS, 4 * q + 4));
                 if (MODE == FM_FWD && pml1 && colq >= 0)
-                    t1 = pml_fwd_m(pm0, a.mvo[0], idx_x(a, colq, y, kk), tab4(XT(T_A_HALF), x), tab4(XT(T_B_HALF), x), t1, wr1);
+                    t1 = pml_fwd_m(pm0, a.mvo[0], ox, tab4(XT(T_A_HALF), x), tab4(XT(T_B_HALF), x), t1, wr1);
                 if (MODE == FM_ADJ && pml1 && exa == 0) t1 = t1 + dpx(ld2s(SC1, 4 * uq - 2), ld4s(SC1, uq), ld2s(SC1, 4 * uq + 4));
                 const float4 rxp = shl1(r0, PR[4 * uq + 4]), axp = shl1(a0, PA[4 * uq + 4]);
                 mbar_wait(&barU[it & 3], (it >> 2) & 1);
@@ -244,10 +259,10 @@ __device__ __forceinline__ void acoustic_brick(float* __restrict__ sm, const CUt
                 const float4 yb = ld4s(PS, q - 10), yc = ld4s(PS, q + 10), yd = ld4s(PS, q + 20);
                 float4 t2 = d4(yb, cs, yc, yd);
                 if (MODE == FM_FWD && pml1 && prow >= 0)
-                    t2 = pml_fwd_m(pm1, a.mvo[4], idx_y(a, x, prow, kk), YT(T_A_HALF)[y], YT(T_B_HALF)[y], t2, wr1);
+                    t2 = pml_fwd_m(pm1, a.mvo[4], oy, YT(T_A_HALF)[y], YT(T_B_HALF)[y], t2, wr1);
                 if (MODE == FM_ADJ && pml1) {
                     if (yex) t2 = t2 + d4(ld4s(SC1, uq - 10), ld4s(SC1, uq), ld4s(SC1, uq + 10), ld4s(SC1, uq + 20));
-                    else if (neary) t2 = t2 + adj_y(a, a.mvi[13], a.mvo[13], YT(T_A_INT), YT(T_B_INT), x, y - 1, kk, 1, yb, cs, yc, yd, wr1 && exa != 1);
+                    else if (neary) t2 = t2 + adj_y3(a, a.mvi[13], a.mvo[13], YT(T_A_INT), YT(T_B_INT), oyb, a.nxq, y - 1, 1, yb, cs, yc, yd, wr1 && exa != 1);
                 }
                 const float4 ryp = ld4s(PR, uq + 10), ayp = ld4s(PA, uq + 10);
                 n2 = fma4(fma4(mh, a0 + ayp, one), *reinterpret_cast<const float4*>(R2), (kB * rcp4(r0 + ryp)) * t2);
@@ -255,13 +270,13 @@ __device__ __forceinline__ void acoustic_brick(float* __restrict__ sm, const CUt
             {   // ---- u3 at (x, y, z+1/2): D+z s
                 float4 t3 = d4(w33b, w33c, w33d, f33);
                 if (MODE == FM_FWD && pml1 && pz >= 0)
-                    t3 = pml_fwd_m(pm2, a.mvo[8], idx_z(a, x, y, pz), ZT(T_A_HALF)[kk & (FT_ZRING - 1)], ZT(T_B_HALF)[kk & (FT_ZRING - 1)], t3, wr1);
+                    t3 = pml_fwd_m(pm2, a.mvo[8], ozq + pz * szp, ZT(T_A_HALF)[kk & (FT_ZRING - 1)], ZT(T_B_HALF)[kk & (FT_ZRING - 1)], t3, wr1);
                 if (MODE == FM_ADJ && pml1 && bz)
-                    t3 = t3 + adj_z(a, a.mvi[17], a.mvo[17], ZT(T_A_INT), ZT(T_B_INT), x, y, kk - 1, 1, w33b, w33c, w33d, f33, wr1);
+                    t3 = t3 + adj_z3(a, a.mvi[17], a.mvo[17], ZT(T_A_INT), ZT(T_B_INT), ozq, szp, kk - 1, 1, w33b, w33c, w33d, f33, wr1);
                 const float4 rzp = ld4s(Rbase + s3n * FT_RPL, uq), azp = ld4s(Abase + s3n * FT_RPL, uq);
                 n3 = fma4(fma4(mh, a0 + azp, one), *reinterpret_cast<const float4*>(R3), (kB * rcp4(r0 + rzp)) * t3);
             }
-            if (edge_xy || !zin) {
+            if (EDGE && (edge_xy || !zin)) {
                 if (!(zin && m0)) { n1.x = 0.0f; n2.x = 0.0f; n3.x = 0.0f; }
                 if (!(zin && m1)) { n1.y = 0.0f; n2.y = 0.0f; n3.y = 0.0f; }
                 if (!(zin && m2)) { n1.z = 0.0f; n2.z = 0.0f; n3.z = 0.0f; }
@@ -273,9 +288,9 @@ __device__ __forceinline__ void acoustic_brick(float* __restrict__ sm, const CUt
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             const long long g = (long long)kk * a.sz + gxy;
             if (wr1) {
-                store_quad(a.out + U1 * box + g, n1, x, a.nx);
-                store_quad(a.out + U2 * box + g, n2, x, a.nx);
-                store_quad(a.out + U3 * box + g, n3, x, a.nx);
+                store_quad<EDGE>(a.out + U1 * box + g, n1, x, a.nx);
+                store_quad<EDGE>(a.out + U2 * box + g, n2, x, a.nx);
+                store_quad<EDGE>(a.out + U3 * box + g, n3, x, a.nx);
             }
         }
         // forward C-PML: psi11, psi22, psi33 of the quad at plane ks = kk - 2, issued ahead of the barrier
@@ -285,9 +300,16 @@ __device__ __forceinline__ void acoustic_brick(float* __restrict__ sm, const CUt
                 const bool ok = inner && it >= 4;
                 const int pzk = ok ? yzslab_row(kk - 2, a.nz, a.P) : -1;
                 const bool ex = ok && colq >= 0, ey = ok && prow >= 0, ez = pzk >= 0;
-                ldg4_into(qm0, a.mvi[9] + (ex ? idx_x(a, colq, y, kk - 2) : 0), ex);
-                ldg4_into(qm1, a.mvi[13] + (ey ? idx_y(a, x, prow, kk - 2) : 0), ey);
-                ldg4_into(qm2, a.mvi[17] + (ez ? idx_z(a, x, y, pzk) : 0), ez);
+                ldg4_into(qm0, a.mvi[9] + (ex ? ox - 2 * sxp : 0), ex);
+                ldg4_into(qm1, a.mvi[13] + (ey ? oy - 2 * syp : 0), ey);
+                ldg4_into(qm2, a.mvi[17] + (ez ? ozq + pzk * szp : 0), ez);
+#if FT_PFMV > 0
+                const bool zpf = kk - 2 + FT_PFMV < a.nz;
+                prefetch_l2(a.mvi[9] + (ox + (FT_PFMV - 2) * sxp), ex && zpf);
+                prefetch_l2(a.mvi[13] + (oy + (FT_PFMV - 2) * syp), ey && zpf);
+                const int pzf = yzslab_row(kk - 2 + FT_PFMV, a.nz, a.P);
+                if (pzf >= 0) prefetch_l2(a.mvi[17] + (ozq + pzf * szp), ok);
+#endif
             }
         }
         float4 e2 = z4;
@@ -296,7 +318,7 @@ __device__ __forceinline__ void acoustic_brick(float* __restrict__ sm, const CUt
         if (MODE == FM_ADJ && exa >= 0 && it >= 4) {
             const bool ok = pok && (unsigned)(kk - 2) < (unsigned)a.nz;
             se2 = ok && (exa == 0 ? colq >= 0 : prow >= 0);
-            i2 = se2 ? (exa == 0 ? idx_x(a, colq, y, kk - 2) : idx_y(a, x, prow, kk - 2)) : 0;
+            i2 = se2 ? (exa == 0 ? ox - 2 * sxp : oy - 2 * syp) : 0;
             ldg4_into(e2, a.mvi[4 * exa] + i2, se2);
         }
         if (pml && tid >= 360 && tid < 364) {
@@ -350,33 +372,34 @@ __device__ __forceinline__ void acoustic_brick(float* __restrict__ sm, const CUt
             {   // D-x u1
                 e11 = dmx(ld2s(U1p + p0, 4 * uq - 2), ld4s(U1p + p0, uq), ld2s(U1p + p0, 4 * uq + 4));
                 if (MODE == FM_FWD && pml2 && colq >= 0)
-                    e11 = pml_fwd_m(qm0, a.mvo[9], idx_x(a, colq, y, ks), tab4(XT(T_A_INT), x), tab4(XT(T_B_INT), x), e11, true);
+                    e11 = pml_fwd_m(qm0, a.mvo[9], ox - 2 * sxp, tab4(XT(T_A_INT), x), tab4(XT(T_B_INT), x), e11, true);
                 if (MODE == FM_ADJ && pml2 && exa == 0) e11 = e11 + dmx(ld2s(SC2, 4 * uq - 2), ld4s(SC2, uq), ld2s(SC2, 4 * uq + 4));
             }
             {   // D-y u2
                 const float4 ya = ld4s(U2p + p0, uq - 20), yb = ld4s(U2p + p0, uq - 10), c = ld4s(U2p + p0, uq), yd = ld4s(U2p + p0, uq + 10);
                 e22 = d4(ya, yb, c, yd);
                 if (MODE == FM_FWD && pml2 && prow >= 0)
-                    e22 = pml_fwd_m(qm1, a.mvo[13], idx_y(a, x, prow, ks), YT(T_A_INT)[y], YT(T_B_INT)[y], e22, true);
+                    e22 = pml_fwd_m(qm1, a.mvo[13], oy - 2 * syp, YT(T_A_INT)[y], YT(T_B_INT)[y], e22, true);
                 if (MODE == FM_ADJ && pml2) {
                     if (exa == 1) e22 = e22 + d4(ld4s(SC2, uq - 20), ld4s(SC2, uq - 10), ld4s(SC2, uq), ld4s(SC2, uq + 10));
-                    else if (neary) e22 = e22 + adj_y(a, a.mvi[4], a.mvo[4], YT(T_A_HALF), YT(T_B_HALF), x, y - 2, ks, 2, ya, yb, c, yd, true);
+                    else if (neary) e22 = e22 + adj_y3(a, a.mvi[4], a.mvo[4], YT(T_A_HALF), YT(T_B_HALF), oyb - 2 * syp, a.nxq, y - 2, 2, ya, yb, c, yd, true);
                 }
             }
             {   // D-z u3
                 const float4 zd = ld4s(U3p + pp1, uq);
                 e33 = d4(u3m2, u3m1, cc3, zd);
                 if (MODE == FM_FWD && pml2 && pz >= 0)
-                    e33 = pml_fwd_m(qm2, a.mvo[17], idx_z(a, x, y, pz), ZT(T_A_INT)[ks & (FT_ZRING - 1)], ZT(T_B_INT)[ks & (FT_ZRING - 1)], e33, true);
+                    e33 = pml_fwd_m(qm2, a.mvo[17], ozq + pz * szp, ZT(T_A_INT)[ks & (FT_ZRING - 1)], ZT(T_B_INT)[ks & (FT_ZRING - 1)], e33, true);
                 if (MODE == FM_ADJ && pml2 && bz)
-                    e33 = e33 + adj_z(a, a.mvi[8], a.mvo[8], ZT(T_A_HALF), ZT(T_B_HALF), x, y, ks - 2, 2, u3m2, u3m1, cc3, zd, true);
+                    e33 = e33 + adj_z3(a, a.mvi[8], a.mvo[8], ZT(T_A_HALF), ZT(T_B_HALF), ozq, szp, ks - 2, 2, u3m2, u3m1, cc3, zd, true);
             }
             const float4 lam = ld4s(sm + AC_OFF_LAM + (it & 1) * FT_LPL, lq);
             const float4 ldiv = (kL * lam) * (e11 + e22 + e33);
             const float4 ns = ld4s(sm + AC_OFF_SO + (it & 1) * FT_LPL, lq) + ldiv;
-            store_quad(a.out + S11 * box + (long long)ks * a.sz + gxy, ns, x, a.nx);
+            store_quad<EDGE>(a.out + S11 * box + (long long)ks * a.sz + gxy, ns, x, a.nx);
         }
         u3m2 = u3m1; u3m1 = cc3;
+        if (MODE != FM_PLAIN) { ox += sxp; oy += syp; oyb += syp; }
         w33a = w33b; w33b = w33c; w33c = w33d; w33d = f33;
     }
 }
@@ -398,8 +421,9 @@ k_step_acoustic(const __grid_constant__ CUtensorMap tmS40, const __grid_constant
         const int b = *s_next;
         if (b >= n) break;
         const int4 wk = __ldg(a.work + a.work_begin + b);
-        if (MODE != FM_PLAIN && (wk.x & FT_WORK_SLAB)) acoustic_brick<MODE>(sm, tmS40, tmS36, tmM37, tmL, tmS32, a, wk, first);
-        else acoustic_brick<FM_PLAIN>(sm, tmS40, tmS36, tmM37, tmL, tmS32, a, wk, first);
+        if (MODE != FM_PLAIN && (wk.x & FT_WORK_SLAB)) acoustic_brick<MODE, true>(sm, tmS40, tmS36, tmM37, tmL, tmS32, a, wk, first);
+        else if (wk.x & FT_WORK_NOEDGE) acoustic_brick<FM_PLAIN, false>(sm, tmS40, tmS36, tmM37, tmL, tmS32, a, wk, first);
+        else acoustic_brick<FM_PLAIN, true>(sm, tmS40, tmS36, tmM37, tmL, tmS32, a, wk, first);
         first = false;
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncthreads();
