@@ -65,3 +65,31 @@ def test_no_oracle_in_product_path():
         if f.suffix in (".py", ".c"):
             t = f.read_text()
             assert "binding" not in t and "libpact" not in t and "ctypes.CDLL(\"libpact" not in t, f
+
+
+def test_sass_uses_tma_mbarriers_and_tensor_memory(pact_lib):
+    """The built library's step kernels carry the sm_100a instructions the design rests on:
+    TMA tensor loads completing on mbarriers, tensor-memory stores / loads (tcgen05.st / ld) and packed fp32 math —
+    and nothing was compiled for another architecture."""
+    import shutil
+    import subprocess
+    from paper_1709_02733_b200 import build
+    tool = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not Path(tool).exists():
+        pytest.skip("cuobjdump not installed")
+    sass = subprocess.run([tool, "-sass", str(build.LIB)], capture_output=True, text=True, check=True).stdout
+    archs = set(re.findall(r"arch = (sm_\w+)", sass))
+    assert archs == {"sm_100a"}, archs
+    kernels = {}
+    for chunk in sass.split("Function : ")[1:]:
+        name = chunk.split("\n", 1)[0].strip()
+        kernels[name] = chunk
+    step = {n: c for n, c in kernels.items() if "k_step" in n}
+    assert len(step) == 6, sorted(step)                      # elastic and fluid-only, C-PML-free / forward / adjoint
+    for n, c in step.items():
+        assert c.count("UTMALDG") >= 10, n                   # cp.async.bulk.tensor
+        assert "SYNCS.ARRIVE.TRANS64" in c and "SYNCS.PHASECHK" in c, n      # mbarrier expect_tx / try_wait
+        assert "FFMA2" in c, n                               # packed f32x2 arithmetic
+    for n, c in step.items():
+        if "acoustic" not in n:                              # elastic step kernels: tensor memory as per-thread scratch
+            assert "STTM" in c and "LDTM" in c, n
