@@ -74,7 +74,15 @@
 #define FT_WT_PLAIN 0
 #endif
 #define FT_WT(MODE) ((MODE) == FM_PLAIN ? FT_WT_PLAIN : FT_WT_PML)
-#define FT_TM_WARP 100                // columns per warp: parked old stresses 36 | s13 ring 16 | s23 ring 16 | s33 ring 32
+// Adjoint, z slabs (FT_ZX 1, needs WT): the filtered increment X = a T of a plane is computed once, when the plane enters
+// the z window as its newest tap (one load of the old T, requested at the top of the iteration), and kept in a TMEM ring
+// of four planes per term ; the other three taps of the transposed recursion come from that ring instead of three more
+// loads per term and plane whose latency sat in front of every use.  Stage 1 terms (sigma13, sigma23, sigma33).
+#ifndef FT_ZX
+#define FT_ZX 1
+#endif
+#define FT_TM_WARP 148                // (with the three X rings of 16 columns)
+#define FT_TM_WARP_OLD 100                // columns per warp: parked old stresses 36 | s13 ring 16 | s23 ring 16 | s33 ring 32
 #define FT_TMEM_COLS_X 512
 #define FT_TMEM_COLS 128              // tensor-memory columns allocated per CTA (mode 2): 3 warps per lane quarter x 36
 
@@ -542,6 +550,8 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
     const bool tmw = SOM == 2 && (WT || tid < 352);
     const uint32_t tm0 = tmem_base + ((uint32_t)((tid >> 5) & 3) << 21) + (uint32_t)(tid >> 7) * (WT ? FT_TM_WARP : 36u);
     const uint32_t tW13 = tm0 + 36u, tW23 = tm0 + 52u, tW33 = tm0 + 68u;      // WT: ring slots of 4 columns, plane j -> j & 3 (s33: j & 7)
+    constexpr bool ZX = FT_ZX != 0 && WT && MODE == FM_ADJ;
+    const uint32_t tXZ = tm0 + 100u;      // ZX: X rings of sigma13, sigma23, sigma33 (16 columns each), plane j -> j & 3
     const int mq = (r - 2) * 9 + (qx - 1);  // quad index in a mu plane (inner threads)
     // own-column global loads are legal where the padded box has storage
     const bool ld_ok = act1 && (!EDGE || ((y + PACT_HALO_Y < a.ny + 2 * PACT_HALO_Y) && (x + 3 + PACT_HALO_X < (int)a.sy)));
@@ -691,6 +701,23 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             tmem_st4(tW13 + 8u, w13a); tmem_st4(tW13 + 12u, w13b); tmem_st4(tW13, w13c);
             tmem_st4(tW23 + 8u, w23a); tmem_st4(tW23 + 12u, w23b); tmem_st4(tW23, w23c);
             tmem_st4(tW33 + 24u, w33a); tmem_st4(tW33 + 28u, w33b); tmem_st4(tW33, w33c); tmem_st4(tW33 + 4u, w33d);
+            if (ZX && pml) {     // X of the three planes below the newest taps of iteration 0: planes -2 .. 0 (sigma33: -1 .. 1), not owned
+                const float4 sv[3][3] = {{w13a, w13b, w13c}, {w23a, w23b, w23c}, {w33b, w33c, w33d}};
+#pragma unroll
+                for (int cc = 0; cc < 3; ++cc)
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) {
+                        const int j = k - 2 + (cc == 2 ? 1 : 0), z = zb - 2 + j;
+                        const int p = yzslab_row(z, a.nz, a.P);
+                        const bool in = pok && p >= 0;
+                        float4 T = f4(0.0f);
+                        ldg4_into(T, a.mgi[5] + 4 * cc + (in ? ozq + p * szp : 0), in);
+                        const float* ztp = sm + OFF_ZT;
+                        const float bk = ztp[(cc == 2 ? T_B_INT : T_B_HALF) * FT_ZRING + (z & (FT_ZRING - 1))];
+                        const float ak = in ? ztp[(cc == 2 ? T_A_INT : T_A_HALF) * FT_ZRING + (z & (FT_ZRING - 1))] : 0.0f;
+                        tmem_st4(tXZ + 16u * cc + 4u * (j & 3), ak * fma4(bk, T, sv[cc][k]));
+                    }
+            }
             tmem_wait_st();
         }
     }
@@ -760,6 +787,21 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
 #endif
             }
         }
+        // ZX: old T of the planes that enter the z windows in this iteration (sigma13, sigma23: kk + 1 ; sigma33: kk + 2)
+        float4 zT[3];
+        bool zin_[2] = {false, false};
+        int zo[2] = {0, 0};
+        const bool bzm = ZX && pml && (kk - 3 < a.P || kk + 5 >= a.nz - 1 - a.P);     // a tap of this or a later plane may lie in a z slab
+        if (ZX) {
+            zT[0] = zT[1] = zT[2] = f4(0.0f);
+            if (bzm) {
+                const int p1 = yzslab_row(kk + 1, a.nz, a.P), p2 = yzslab_row(kk + 2, a.nz, a.P);
+                zin_[0] = pok && p1 >= 0; zin_[1] = pok && p2 >= 0;
+                zo[0] = zin_[0] ? ozq + p1 * szp : 0; zo[1] = zin_[1] ? ozq + p2 * szp : 0;
+                ldg4_into(zT[0], a.mgi[5] + zo[0], zin_[0]); ldg4_into(zT[1], a.mgi[5] + 4 + zo[0], zin_[0]);
+                ldg4_into(zT[2], a.mgi[5] + 8 + zo[1], zin_[1]);
+            }
+        }
         mbar_wait(&barG[it & 1], (it >> 1) & 1);
 
         const int s3 = it % 3, s3n = (it + 1) % 3;
@@ -818,6 +860,37 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             if (WT) {
                 tmem_st4(tW13 + 4u * ((it + 1) & 3), f13); tmem_st4(tW23 + 4u * ((it + 1) & 3), f23); tmem_st4(tW33 + 4u * ((it + 2) & 7), f33);
             }
+            // ZX: T <- b T + s and X = a T of the entering planes ; T is stored by the brick that owns the plane
+            float4 zX[3];
+            if (ZX) {
+                zX[0] = zX[1] = zX[2] = f4(0.0f);
+                if (bzm) {
+                    const int z1 = kk + 1, z2 = kk + 2;
+                    const bool w1 = inner && zin_[0] && z1 >= zb && z1 < ze, w2 = inner && zin_[1] && z2 >= zb && z2 < ze;
+                    const float b1h = ZT(T_B_HALF)[z1 & (FT_ZRING - 1)], a1h = zin_[0] ? ZT(T_A_HALF)[z1 & (FT_ZRING - 1)] : 0.0f;
+                    const float b2i = ZT(T_B_INT)[z2 & (FT_ZRING - 1)], a2i = zin_[1] ? ZT(T_A_INT)[z2 & (FT_ZRING - 1)] : 0.0f;
+                    const float4 Ta = fma4(b1h, zT[0], f13), Tb = fma4(b1h, zT[1], f23), Tc = fma4(b2i, zT[2], f33);
+                    if (w1) { stg4(a.mgo[5] + zo[0], Ta); stg4(a.mgo[5] + 4 + zo[0], Tb); }
+                    if (w2) stg4(a.mgo[5] + 8 + zo[1], Tc);
+                    zX[0] = a1h * Ta; zX[1] = a1h * Tb; zX[2] = a2i * Tc;
+                    tmem_st4(tXZ + 4u * ((it + 1) & 3), zX[0]); tmem_st4(tXZ + 16u + 4u * ((it + 1) & 3), zX[1]);
+                    tmem_st4(tXZ + 32u + 4u * ((it + 2) & 3), zX[2]);
+                }
+            }
+            // ZX: the z differences of X (taps kk - 2 .. kk + 1 ; sigma33: kk - 1 .. kk + 2), three taps from the rings.  Warp-wide
+            // tensor-memory loads: under the CTA-uniform test only.
+            float4 zD[3];
+            if (ZX) {
+                zD[0] = zD[1] = zD[2] = f4(0.0f);
+                if (pml && (kk - 2 < a.P || kk + 2 >= a.nz - 1 - a.P)) {
+                    const uint32_t s2 = 4u * ((it + 2) & 3), s3_ = 4u * ((it + 3) & 3), s0 = 4u * (it & 3), s1 = 4u * ((it + 1) & 3);
+                    const float4 xa0 = tmem_ld4(tXZ + s2), xb0 = tmem_ld4(tXZ + s3_), xc0 = tmem_ld4(tXZ + s0);
+                    const float4 xa1 = tmem_ld4(tXZ + 16u + s2), xb1 = tmem_ld4(tXZ + 16u + s3_), xc1 = tmem_ld4(tXZ + 16u + s0);
+                    const float4 xa2 = tmem_ld4(tXZ + 32u + s3_), xb2 = tmem_ld4(tXZ + 32u + s0), xc2 = tmem_ld4(tXZ + 32u + s1);
+                    tmem_wait_ld();
+                    zD[0] = d4(xa0, xb0, xc0, zX[0]); zD[1] = d4(xa1, xb1, xc1, zX[1]); zD[2] = d4(xa2, xb2, xc2, zX[2]);
+                }
+            }
 
             const bool wr1 = inner && kk >= zb && kk < ze;          // this CTA owns u(x..x+3, y, kk)
             // C-PML at this plane: z slab position of kk ; is any tap of the thread inside a slab
@@ -857,7 +930,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                     if (exa == 0) t1 = t1 + dpx(ld2s(S, 4 * uq - 2), ld4s(S, uq), ld2s(S, 4 * uq + 4));
                     if (yex) t2 = t2 + d4(ld4s(S, uq - 20), ld4s(S, uq - 10), ld4s(S, uq), ld4s(S, uq + 10));
                     else if (neary) t2 = t2 + adj_y3(a, a.mgi[4], a.mgo[4], YT(T_A_HALF), YT(T_B_HALF), oyb, rsy, y - 2, 2, ya, yb, c12, yd, wr1 && exa != 1);
-                    if (bz) t3 = t3 + adj_z3(a, a.mgi[5], a.mgo[5], ZT(T_A_HALF), ZT(T_B_HALF), ozq, szp, kk - 2, 2, w13a, w13b, w13c, f13, wr1);
+                    if (bz) t3 = t3 + (ZX ? zD[0] : adj_z3(a, a.mgi[5], a.mgo[5], ZT(T_A_HALF), ZT(T_B_HALF), ozq, szp, kk - 2, 2, w13a, w13b, w13c, f13, wr1));
                 }
                 const float4 rxp = shl1(r0, PR[4 * uq + 4]), axp = shl1(a0, PA[4 * uq + 4]);
                 mbar_wait(&barU[it & 1], (it >> 1) & 1);      // u_old(kk) has landed in the ring slot
@@ -882,7 +955,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                     if (exa == 0) t1 = t1 + dmx(ld2s(S, 4 * uq - 2), ld4s(S, uq), ld2s(S, 4 * uq + 4));
                     if (yex) t2 = t2 + d4(ld4s(S, uq - 10), ld4s(S, uq), ld4s(S, uq + 10), ld4s(S, uq + 20));
                     else if (neary) t2 = t2 + adj_y3(a, a.mgi[4] + 4, a.mgo[4] + 4, YT(T_A_INT), YT(T_B_INT), oyb, rsy, y - 1, 1, yb, c22, yc, yd, wr1 && exa != 1);
-                    if (bz) t3 = t3 + adj_z3(a, a.mgi[5] + 4, a.mgo[5] + 4, ZT(T_A_HALF), ZT(T_B_HALF), ozq, szp, kk - 2, 2, w23a, w23b, w23c, f23, wr1);
+                    if (bz) t3 = t3 + (ZX ? zD[1] : adj_z3(a, a.mgi[5] + 4, a.mgo[5] + 4, ZT(T_A_HALF), ZT(T_B_HALF), ozq, szp, kk - 2, 2, w23a, w23b, w23c, f23, wr1));
                 }
                 const float4 ryp = ld4s(PR, uq + 10), ayp = ld4s(PA, uq + 10);
                 n2 = fma4(fma4(mh, a0 + ayp, one), *reinterpret_cast<const float4*>(R2), (kB * rcp4(r0 + ryp)) * (t1 + t2 + t3));
@@ -905,7 +978,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                     if (exa == 0) t1 = t1 + dmx(ld2s(S, 4 * uq - 2), ld4s(S, uq), ld2s(S, 4 * uq + 4));
                     if (yex) t2 = t2 + d4(ld4s(S, uq - 20), ld4s(S, uq - 10), ld4s(S, uq), ld4s(S, uq + 10));
                     else if (neary) t2 = t2 + adj_y3(a, a.mgi[4] + 8, a.mgo[4] + 8, YT(T_A_HALF), YT(T_B_HALF), oyb, rsy, y - 2, 2, ya, yb, w23c, yd, wr1 && exa != 1);
-                    if (bz) t3 = t3 + adj_z3(a, a.mgi[5] + 8, a.mgo[5] + 8, ZT(T_A_INT), ZT(T_B_INT), ozq, szp, kk - 1, 1, w33b, w33c, w33d, f33, wr1);
+                    if (bz) t3 = t3 + (ZX ? zD[2] : adj_z3(a, a.mgi[5] + 8, a.mgo[5] + 8, ZT(T_A_INT), ZT(T_B_INT), ozq, szp, kk - 1, 1, w33b, w33c, w33d, f33, wr1));
                 }
                 const float4 rzp = ld4s(Rbase + s3n * FT_RPL, uq), azp = ld4s(Abase + s3n * FT_RPL, uq);
                 n3 = fma4(fma4(mh, a0 + azp, one), *reinterpret_cast<const float4*>(R3), (kB * rcp4(r0 + rzp)) * (t1 + t2 + t3));
