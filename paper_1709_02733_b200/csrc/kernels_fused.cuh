@@ -81,8 +81,9 @@
 #ifndef FT_ZX
 #define FT_ZX 1
 #endif
-#define FT_TM_WARP 148                // (with the three X rings of 16 columns)
-#define FT_TM_WARP_OLD 100                // columns per warp: parked old stresses 36 | s13 ring 16 | s23 ring 16 | s33 ring 32
+// columns per warp with WT: parked old s11, s22, s12, s33 3 x 16 | s13 ring 16 | s23 ring 16 | s33 ring 16 | X rings of
+// stage 1 3 x 12 | X rings of stage 2 3 x 12  (3 warps per lane quarter: 504 of 512 columns)
+#define FT_TM_WARP 168
 #define FT_TMEM_COLS_X 512
 #define FT_TMEM_COLS 128              // tensor-memory columns allocated per CTA (mode 2): 3 warps per lane quarter x 36
 
@@ -549,9 +550,10 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
     // [plane % 3][s11, s22, s12][4]).  Warp 11 holds no tile quad and takes no part (its u-region lanes diverge).
     const bool tmw = SOM == 2 && (WT || tid < 352);
     const uint32_t tm0 = tmem_base + ((uint32_t)((tid >> 5) & 3) << 21) + (uint32_t)(tid >> 7) * (WT ? FT_TM_WARP : 36u);
-    const uint32_t tW13 = tm0 + 36u, tW23 = tm0 + 52u, tW33 = tm0 + 68u;      // WT: ring slots of 4 columns, plane j -> j & 3 (s33: j & 7)
+    const uint32_t tW13 = tm0 + 48u, tW23 = tm0 + 64u, tW33 = tm0 + 80u;      // WT: ring slots of 4 columns, plane j -> j & 3
+    constexpr uint32_t SOS = WT ? 16u : 12u;      // columns per parking slot (WT: the old s33 is parked as well)
     constexpr bool ZX = FT_ZX != 0 && WT && MODE == FM_ADJ;
-    const uint32_t tXZ = tm0 + 100u;      // ZX: X rings of sigma13, sigma23, sigma33 (16 columns each), plane j -> j & 3
+    const uint32_t tXZ = tm0 + 96u;       // ZX: X rings of sigma13, sigma23, sigma33 (12 columns each), plane j -> j mod 3
     const int mq = (r - 2) * 9 + (qx - 1);  // quad index in a mu plane (inner threads)
     // own-column global loads are legal where the padded box has storage
     const bool ld_ok = act1 && (!EDGE || ((y + PACT_HALO_Y < a.ny + 2 * PACT_HALO_Y) && (x + 3 + PACT_HALO_X < (int)a.sy)));
@@ -700,7 +702,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
         if (WT) {      // planes -2, -1, 0 (s33: and 1) of the rings
             tmem_st4(tW13 + 8u, w13a); tmem_st4(tW13 + 12u, w13b); tmem_st4(tW13, w13c);
             tmem_st4(tW23 + 8u, w23a); tmem_st4(tW23 + 12u, w23b); tmem_st4(tW23, w23c);
-            tmem_st4(tW33 + 24u, w33a); tmem_st4(tW33 + 28u, w33b); tmem_st4(tW33, w33c); tmem_st4(tW33 + 4u, w33d);
+            tmem_st4(tW33 + 12u, w33b); tmem_st4(tW33, w33c); tmem_st4(tW33 + 4u, w33d);      // (the oldest entry is parked, not ringed)
             if (ZX && pml) {     // X of the three planes below the newest taps of iteration 0: planes -2 .. 0 (sigma33: -1 .. 1), not owned
                 const float4 sv[3][3] = {{w13a, w13b, w13c}, {w23a, w23b, w23c}, {w33b, w33c, w33d}};
 #pragma unroll
@@ -715,7 +717,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                         const float* ztp = sm + OFF_ZT;
                         const float bk = ztp[(cc == 2 ? T_B_INT : T_B_HALF) * FT_ZRING + (z & (FT_ZRING - 1))];
                         const float ak = in ? ztp[(cc == 2 ? T_A_INT : T_A_HALF) * FT_ZRING + (z & (FT_ZRING - 1))] : 0.0f;
-                        tmem_st4(tXZ + 16u * cc + 4u * (j & 3), ak * fma4(bk, T, sv[cc][k]));
+                        tmem_st4(tXZ + 12u * cc + 4u * ((j + 3) % 3), ak * fma4(bk, T, sv[cc][k]));
                     }
             }
             tmem_wait_st();
@@ -858,7 +860,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             f23 = ld4s(sm + FT_OFF_S23 + s3n * FT_BOX, q);
             f33 = ld4s(sm + FT_OFF_S33 + (it & 1) * FT_UPL, uq);   // plane kk+2
             if (WT) {
-                tmem_st4(tW13 + 4u * ((it + 1) & 3), f13); tmem_st4(tW23 + 4u * ((it + 1) & 3), f23); tmem_st4(tW33 + 4u * ((it + 2) & 7), f33);
+                tmem_st4(tW13 + 4u * ((it + 1) & 3), f13); tmem_st4(tW23 + 4u * ((it + 1) & 3), f23); tmem_st4(tW33 + 4u * ((it + 2) & 3), f33);
             }
             // ZX: T <- b T + s and X = a T of the entering planes ; T is stored by the brick that owns the plane
             float4 zX[3];
@@ -873,8 +875,6 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                     if (w1) { stg4(a.mgo[5] + zo[0], Ta); stg4(a.mgo[5] + 4 + zo[0], Tb); }
                     if (w2) stg4(a.mgo[5] + 8 + zo[1], Tc);
                     zX[0] = a1h * Ta; zX[1] = a1h * Tb; zX[2] = a2i * Tc;
-                    tmem_st4(tXZ + 4u * ((it + 1) & 3), zX[0]); tmem_st4(tXZ + 16u + 4u * ((it + 1) & 3), zX[1]);
-                    tmem_st4(tXZ + 32u + 4u * ((it + 2) & 3), zX[2]);
                 }
             }
             // ZX: the z differences of X (taps kk - 2 .. kk + 1 ; sigma33: kk - 1 .. kk + 2), three taps from the rings.  Warp-wide
@@ -882,13 +882,16 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             float4 zD[3];
             if (ZX) {
                 zD[0] = zD[1] = zD[2] = f4(0.0f);
+                const uint32_t q0 = 4u * (uint32_t)s3, q1 = 4u * (uint32_t)s3n, q2 = 4u * (uint32_t)((it + 2) % 3);    // planes it, it + 1 (= it - 2), it + 2 (= it - 1)
                 if (pml && (kk - 2 < a.P || kk + 2 >= a.nz - 1 - a.P)) {
-                    const uint32_t s2 = 4u * ((it + 2) & 3), s3_ = 4u * ((it + 3) & 3), s0 = 4u * (it & 3), s1 = 4u * ((it + 1) & 3);
-                    const float4 xa0 = tmem_ld4(tXZ + s2), xb0 = tmem_ld4(tXZ + s3_), xc0 = tmem_ld4(tXZ + s0);
-                    const float4 xa1 = tmem_ld4(tXZ + 16u + s2), xb1 = tmem_ld4(tXZ + 16u + s3_), xc1 = tmem_ld4(tXZ + 16u + s0);
-                    const float4 xa2 = tmem_ld4(tXZ + 32u + s3_), xb2 = tmem_ld4(tXZ + 32u + s0), xc2 = tmem_ld4(tXZ + 32u + s1);
+                    const float4 xa0 = tmem_ld4(tXZ + q1), xb0 = tmem_ld4(tXZ + q2), xc0 = tmem_ld4(tXZ + q0);
+                    const float4 xa1 = tmem_ld4(tXZ + 12u + q1), xb1 = tmem_ld4(tXZ + 12u + q2), xc1 = tmem_ld4(tXZ + 12u + q0);
+                    const float4 xa2 = tmem_ld4(tXZ + 24u + q2), xb2 = tmem_ld4(tXZ + 24u + q0), xc2 = tmem_ld4(tXZ + 24u + q1);
                     tmem_wait_ld();
                     zD[0] = d4(xa0, xb0, xc0, zX[0]); zD[1] = d4(xa1, xb1, xc1, zX[1]); zD[2] = d4(xa2, xb2, xc2, zX[2]);
+                }
+                if (bzm) {      // the entering planes take the slots of the planes that just left the windows (read above)
+                    tmem_st4(tXZ + q1, zX[0]); tmem_st4(tXZ + 12u + q1, zX[1]); tmem_st4(tXZ + 24u + q2, zX[2]);
                 }
             }
 
@@ -904,7 +907,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             const float4 r0 = ld4s(PR, uq), a0 = ld4s(PA, uq);
             const float4 one = f4(1.0f), mh = f4(-0.5f);
             const float4 c12 = ld4s(P12, q);
-            const uint32_t tms = tm0 + (uint32_t)(it % 3) * 12u;      // SOM 2: this plane's parking columns
+            const uint32_t tms = tm0 + (uint32_t)(it % 3) * SOS;      // SOM 2: this plane's parking columns
             float4 n1, n2, n3;
             const int sl = it % RING;
             float* const R1 = sm + OFF_UR + (0 * RING + sl) * FT_UPL + 4 * uq;
@@ -964,8 +967,9 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                 const float2 l = ld2s(P13, 4 * uq - 2), rr = ld2s(P13, 4 * uq + 4);
                 const float4 ya = ld4s(P23, q - 20), yb = ld4s(P23, q - 10), yd = ld4s(P23, q + 10);
                 if (WT) {
-                    w33b = tmem_ld4(tW33 + 4u * ((it + 7) & 7)); w33c = tmem_ld4(tW33 + 4u * (it & 7)); w33d = tmem_ld4(tW33 + 4u * ((it + 1) & 7));
+                    w33b = tmem_ld4(tW33 + 4u * ((it + 3) & 3)); w33c = tmem_ld4(tW33 + 4u * (it & 3)); w33d = tmem_ld4(tW33 + 4u * ((it + 1) & 3));
                     tmem_wait_ld();
+                    tmem_st4(tms + 12u, w33c);      // s33 of plane kk: the old value stage 2 adds to two iterations on
                 }
                 float4 t1 = dmx(l, w13c, rr), t2 = d4(ya, yb, w23c, yd), t3 = d4(w33b, w33c, w33d, f33);
                 if (MODE == FM_FWD && slab1) {
@@ -1048,13 +1052,28 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
         // oldest window entries.  Warp-wide instructions, hence outside the divergent block of stage 2 ; requested here, ahead
         // of the block barrier, and waited for at the top of stage 2.
         float4 so11 = z4, so22 = z4, so12 = z4;
+        // ZX, stage 2: old T' of the u planes that enter the z taps of the stress update (u1, u2: plane kk ; u3: plane kk - 1)
+        float4 yT[3];
+        bool yin_[2] = {false, false};
+        int yo[2] = {0, 0};
+        const bool bzm2 = ZX && pml && it >= 1 && (kk - 4 < a.P || kk + 5 >= a.nz - 1 - a.P);
+        if (ZX) {
+            yT[0] = yT[1] = yT[2] = f4(0.0f);
+            if (bzm2) {
+                const int p1 = yzslab_row(kk, a.nz, a.P), p2 = yzslab_row(kk - 1, a.nz, a.P);
+                yin_[0] = inner && p1 >= 0; yin_[1] = inner && p2 >= 0;
+                yo[0] = yin_[0] ? ozq + p1 * szp : 0; yo[1] = yin_[1] ? ozq + p2 * szp : 0;
+                ldg4_into(yT[0], a.mgi[2] + yo[0], yin_[0]); ldg4_into(yT[1], a.mgi[2] + 4 + yo[0], yin_[0]);
+                ldg4_into(yT[2], a.mgi[2] + 8 + yo[1], yin_[1]);
+            }
+        }
         if ((WT || tmw) && it >= 4) {
             if (tmw) {
-                const uint32_t tml = tm0 + (uint32_t)((it + 1) % 3) * 12u;     // plane it - 2
+                const uint32_t tml = tm0 + (uint32_t)((it + 1) % 3) * SOS;     // plane it - 2
                 so11 = tmem_ld4(tml); so22 = tmem_ld4(tml + 4u); so12 = tmem_ld4(tml + 8u);
             }
             if (WT) {   // old s13, s23, s33 of plane ks = the oldest window entries
-                w13a = tmem_ld4(tW13 + 4u * ((it + 2) & 3)); w23a = tmem_ld4(tW23 + 4u * ((it + 2) & 3)); w33a = tmem_ld4(tW33 + 4u * ((it + 6) & 7));
+                w13a = tmem_ld4(tW13 + 4u * ((it + 2) & 3)); w23a = tmem_ld4(tW23 + 4u * ((it + 2) & 3)); w33a = tmem_ld4(tm0 + (uint32_t)((it + 1) % 3) * SOS + 12u);
             }
         }
         if (WT || tmw) tmem_wait_st();
@@ -1125,6 +1144,37 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
             __syncthreads();
         }
         if ((WT || tmw) && it >= 4) tmem_wait_ld();      // (requested ahead of the block barrier)
+        // ZX, stage 2: T' <- b T' + u and Y = a T' of the entering planes (stored by the brick that owns the plane), the z
+        // differences of Y from the rings (taps ks - 1 .. ks + 2 ; u3: ks - 2 .. ks + 1), then the entering planes take the
+        // slots of the planes that left.  CTA-uniform tests around the warp-wide tensor-memory instructions.
+        float4 yD[3];
+        if (ZX) {
+            yD[0] = yD[1] = yD[2] = f4(0.0f);
+            float4 yX[3];
+            yX[0] = yX[1] = yX[2] = f4(0.0f);
+            const uint32_t tYZ = tm0 + 132u;
+            const uint32_t q0 = 4u * (uint32_t)(it % 3), q1 = 4u * (uint32_t)((it + 1) % 3), q2 = 4u * (uint32_t)((it + 2) % 3);
+            if (bzm2) {
+                const int z1 = kk, z2 = kk - 1;
+                const float4 v1 = ld4s(sm + OFF_UR + (0 * RING + it % RING) * FT_UPL, uq), v2 = ld4s(sm + OFF_UR + (1 * RING + it % RING) * FT_UPL, uq);
+                const float4 v3 = ld4s(sm + OFF_UR + (2 * RING + (it + RING - 1) % RING) * FT_UPL, uq);
+                const bool w1 = yin_[0] && z1 >= zb && z1 < ze, w2 = yin_[1] && z2 >= zb && z2 < ze;
+                const float b1i = ZT(T_B_INT)[z1 & (FT_ZRING - 1)], a1i = yin_[0] ? ZT(T_A_INT)[z1 & (FT_ZRING - 1)] : 0.0f;
+                const float b2h = ZT(T_B_HALF)[z2 & (FT_ZRING - 1)], a2h = yin_[1] ? ZT(T_A_HALF)[z2 & (FT_ZRING - 1)] : 0.0f;
+                const float4 Ta = fma4(b1i, yT[0], v1), Tb = fma4(b1i, yT[1], v2), Tc = fma4(b2h, yT[2], v3);
+                if (w1) { stg4(a.mgo[2] + yo[0], Ta); stg4(a.mgo[2] + 4 + yo[0], Tb); }
+                if (w2) stg4(a.mgo[2] + 8 + yo[1], Tc);
+                yX[0] = a1i * Ta; yX[1] = a1i * Tb; yX[2] = a2h * Tc;
+            }
+            if (it >= 4 && pml && (kk - 4 < a.P || kk >= a.nz - 1 - a.P)) {      // bz of stage 2 (ks = kk - 2)
+                const float4 xa0 = tmem_ld4(tYZ + q0), xb0 = tmem_ld4(tYZ + q1), xc0 = tmem_ld4(tYZ + q2);                      // planes it - 3, it - 2, it - 1
+                const float4 xa1 = tmem_ld4(tYZ + 12u + q0), xb1 = tmem_ld4(tYZ + 12u + q1), xc1 = tmem_ld4(tYZ + 12u + q2);
+                const float4 xa2 = tmem_ld4(tYZ + 24u + q2), xb2 = tmem_ld4(tYZ + 24u + q0), xc2 = tmem_ld4(tYZ + 24u + q1);    // planes it - 4, it - 3, it - 2
+                tmem_wait_ld();
+                yD[0] = d4(xa0, xb0, xc0, yX[0]); yD[1] = d4(xa1, xb1, xc1, yX[1]); yD[2] = d4(xa2, xb2, xc2, yX[2]);
+            }
+            if (bzm2) { tmem_st4(tYZ + q0, yX[0]); tmem_st4(tYZ + 12u + q0, yX[1]); tmem_st4(tYZ + 24u + q2, yX[2]); }
+        }
         if (inner && it >= 4) {
             const int j = it - 2;             // relative plane of ks
             // SOM 0, 1: old s12(ks) (and s11, s22) by own-column loads (L2 hits: group ks fetched the planes two
@@ -1161,7 +1211,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                     if (exa == 0) e11 = e11 + dmx(ld2s(SC2a, 4 * uq - 2), ld4s(SC2a, uq), ld2s(SC2a, 4 * uq + 4));
                     if (exa == 1) g12 = g12 + d4(ld4s(SC2a, uq - 10), ld4s(SC2a, uq), ld4s(SC2a, uq + 10), ld4s(SC2a, uq + 20));
                     else if (neary) g12 = g12 + adj_y3(a, a.mgi[1], a.mgo[1], YT(T_A_INT), YT(T_B_INT), oyb2, rsy, y - 1, 1, ya, c, yc, yd, true);
-                    if (bz) g13 = g13 + adj_z3(a, a.mgi[2], a.mgo[2], ZT(T_A_INT), ZT(T_B_INT), ozq, szp, ks - 1, 1, za, c, zc, zd, true);
+                    if (bz) g13 = g13 + (ZX ? yD[0] : adj_z3(a, a.mgi[2], a.mgo[2], ZT(T_A_INT), ZT(T_B_INT), ozq, szp, ks - 1, 1, za, c, zc, zd, true));
                 }
             }
             {   // ---- derivatives of u2: D+x (g21), D-y (e22), D+z (g23)
@@ -1179,7 +1229,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                     if (exa == 0) g21 = g21 + dpx(ld2s(SC2b, 4 * uq - 2), ld4s(SC2b, uq), ld2s(SC2b, 4 * uq + 4));
                     if (exa == 1) e22 = e22 + d4(ld4s(SC2b, uq - 20), ld4s(SC2b, uq - 10), ld4s(SC2b, uq), ld4s(SC2b, uq + 10));
                     else if (neary) e22 = e22 + adj_y3(a, a.mgi[1] + 4, a.mgo[1] + 4, YT(T_A_HALF), YT(T_B_HALF), oyb2, rsy, y - 2, 2, ya, yb, c, yd, true);
-                    if (bz) g23 = g23 + adj_z3(a, a.mgi[2] + 4, a.mgo[2] + 4, ZT(T_A_INT), ZT(T_B_INT), ozq, szp, ks - 1, 1, za, c, zc, zd, true);
+                    if (bz) g23 = g23 + (ZX ? yD[1] : adj_z3(a, a.mgi[2] + 4, a.mgo[2] + 4, ZT(T_A_INT), ZT(T_B_INT), ozq, szp, ks - 1, 1, za, c, zc, zd, true));
                 }
             }
             {   // ---- derivatives of u3: D+x (g31), D+y (g32), D-z (e33)
@@ -1197,7 +1247,7 @@ __device__ __forceinline__ void fused_brick(float* __restrict__ sm, const CUtens
                     if (exa == 0) g31 = g31 + dpx(ld2s(SC2c, 4 * uq - 2), ld4s(SC2c, uq), ld2s(SC2c, 4 * uq + 4));
                     if (exa == 1) g32 = g32 + d4(ld4s(SC2c, uq - 10), ld4s(SC2c, uq), ld4s(SC2c, uq + 10), ld4s(SC2c, uq + 20));
                     else if (neary) g32 = g32 + adj_y3(a, a.mgi[1] + 8, a.mgo[1] + 8, YT(T_A_INT), YT(T_B_INT), oyb2, rsy, y - 1, 1, ya, c, yc, yd, true);
-                    if (bz) e33 = e33 + adj_z3(a, a.mgi[2] + 8, a.mgo[2] + 8, ZT(T_A_HALF), ZT(T_B_HALF), ozq, szp, ks - 2, 2, za, zb_, c, zd, true);
+                    if (bz) e33 = e33 + (ZX ? yD[2] : adj_z3(a, a.mgi[2] + 8, a.mgo[2] + 8, ZT(T_A_HALF), ZT(T_B_HALF), ozq, szp, ks - 2, 2, za, zb_, c, zd, true));
                 }
             }
 
