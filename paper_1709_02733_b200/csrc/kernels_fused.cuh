@@ -304,7 +304,13 @@ __device__ __forceinline__ void prefetch_l2(const float* p, bool pred)
 {
     asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %1, 0;\n\t@p prefetch.global.L2 [%0];\n\t}" ::"l"(p), "r"((int)pred) : "memory");
 }
-__device__ __forceinline__ void stg4(float* p, float4 v) { *reinterpret_cast<float4*>(p) = v; }
+// 128-bit store that does not allocate in L1 (st.global.cg): the step kernels leave ~20 KB of L1 beside their shared
+// memory, and the default write-allocating stores of the nine output fields kept evicting what little of it the loads
+// use (interior launch -4 % at 512^3 ; .cs and .wt measured within 1 % of it)
+__device__ __forceinline__ void stg4(float* p, float4 v)
+{
+    asm volatile("st.global.cg.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
 
 // store the in-grid lanes of a quad starting at column x (EDGE = false: the whole quad is in the grid)
 template <bool EDGE = true>
