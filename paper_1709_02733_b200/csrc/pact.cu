@@ -700,7 +700,41 @@ static int build_work(pact_ctx* c)
             }
     };
     std::vector<std::pair<int, int>> bl, bs, il, is, zl, zs;
-    if (!tbd.empty()) cut_chunks(0, g.nz, c->zchunk, LL, LS, bl, bs);
+    // C-PML bricks: the long / short chunk lengths that give the shortest makespan when the launch hands the bricks out
+    // in list order to num_sms CTAs (greedy list scheduling, 7 start-up iterations per brick, corner tiles 1.6 x, other
+    // boundary tiles 1.3 x the cost of a z-slab brick of an interior tile per plane: the adjoint's ratios).  On large
+    // grids this reproduces 128 / 40 ; on small ones (256^3: 28 boundary columns for 148 SMs) one long brick would
+    // otherwise be the whole launch.
+    int LLs = LL, LSs = LS;
+    if (P > 0 && c->zchunk == 0 && c->chunk_long == 0 && c->chunk_short == 0 && !tbd.empty()) {
+        auto weight = [&](const std::pair<int, int>& t) {
+            return (!interior_1d(t.first * FT_TX, g.nx) && !interior_1d(t.second * FT_TY, g.ny)) ? 1.6 : 1.3;
+        };
+        double best = 1e300;
+        const int cl[] = {24, 32, 48, 64, 96, 128}, cs[] = {16, 24, 40};
+        for (int a = 0; a < 6; ++a)
+            for (int b = 0; b < 3; ++b) {
+                if (cs[b] > cl[a]) continue;
+                std::vector<std::pair<int, int>> l1, s1, l2, s2;
+                cut_chunks(0, g.nz, 0, cl[a], cs[b], l1, s1);
+                if (!tin.empty()) { cut_chunks(0, zlo, 0, cl[a], cs[b], l2, s2); cut_chunks(zhi, g.nz, 0, cl[a], cs[b], l2, s2); }
+                std::vector<double> costs;
+                for (auto& ch : l1) for (auto& t : tbd) costs.push_back(weight(t) * (ch.second - ch.first + 7));
+                for (auto& ch : s1) for (auto& t : tbd) costs.push_back(weight(t) * (ch.second - ch.first + 7));
+                for (auto& ch : l2) for (size_t t = 0; t < tin.size(); ++t) costs.push_back(1.0 * (ch.second - ch.first + 7));
+                for (auto& ch : s2) for (size_t t = 0; t < tin.size(); ++t) costs.push_back(1.0 * (ch.second - ch.first + 7));
+                std::vector<double> sm(c->num_sms, 0.0);        // min-heap of the CTAs' finish times
+                auto gt = [](double x, double y) { return x > y; };
+                for (double w : costs) {
+                    std::pop_heap(sm.begin(), sm.end(), gt);
+                    sm.back() += w;
+                    std::push_heap(sm.begin(), sm.end(), gt);
+                }
+                const double mk = *std::max_element(sm.begin(), sm.end());
+                if (mk < best * 0.995) { best = mk; LLs = cl[a]; LSs = cs[b]; }      // (a later candidate must be clearly better)
+            }
+    }
+    if (!tbd.empty()) cut_chunks(0, g.nz, c->zchunk, LLs, LSs, bl, bs);
     if (!tin.empty()) {
         // Interior bricks all cost the same per plane, so equal chunks in a whole number of waves beat the long / short mix:
         // k chunks per column minimising waves x (planes per chunk + 7 start-up iterations).  (512^3, npml 16: 196 columns
@@ -717,8 +751,8 @@ static int build_work(pact_ctx* c)
             cut_chunks(zlo, zhi, (n + best_k - 1) / best_k, 0, 0, il, is);
         }
         if (P > 0) {   // the z slabs of interior tiles: thin bricks
-            cut_chunks(0, zlo, c->zchunk, LL, LS, zl, zs);
-            cut_chunks(zhi, g.nz, c->zchunk, LL, LS, zl, zs);
+            cut_chunks(0, zlo, c->zchunk, LLs, LSs, zl, zs);
+            cut_chunks(zhi, g.nz, c->zchunk, LLs, LSs, zl, zs);
         }
     }
     const int slab = P > 0 ? FT_WORK_SLAB : 0;
